@@ -1,0 +1,167 @@
+/*
+ * grinqh.h — C ABI of the B200-native GRINQH decode hot path.
+ *
+ * Method: GRINQH (arxiv/paper_2606_23419).  Citations are PAPER.md:LINE of the
+ * paper text this build was written from.
+ *
+ *   y[t, n] = sum_k  x[t, k] * w_hat(k, n; b_tk)
+ *
+ * over a bit-planar, nested 8-bit weight store.  Every decode
+ * step each input channel k of the current vector gets a bit width b_k in
+ * {0..8} from the rank of |x_k| (top-p form of :271) and only
+ * the top b_k bit planes of weight row k are fetched; the truncated code is
+ * reconstructed with the paper's midpoint bias
+ *
+ *   w_hat = s * (q_b * 2^(8-b) + phi_b) + z ,   phi_b = 2^(8-b-1)
+ *
+ * with phi_8 = 0 and a b = 0 row contributing exactly nothing (DESIGN.md
+ * readings #5, #7).
+ *
+ * Conventions for every call below
+ *   - "dev" pointers are DEVICE pointers owned by the caller; "host" pointers
+ *     are ordinary host memory.  The library never allocates, frees or keeps a
+ *     pointer after the call returns.
+ *   - Every call only ENQUEUES work on `stream` (a cudaStream_t passed as
+ *     void*; NULL = the legacy default stream).  Nothing synchronises.  All
+ *     device entry points are CUDA-graph capturable.
+ *   - Return value: GRINQH_OK (0) or a negative grinqh_status.  On error
+ *     nothing has been enqueued.
+ *   - W is [K, N] row-major fp16: K = d_in rows (input channels), N = d_out.
+ *     group = 128 consecutive input channels of one output column
+ *     ("group size G=128").  Required: K % 128 == 0, N % 32 == 0,
+ *     1 <= T <= 4, all base pointers 16-byte aligned.
+ *   - Plane j (j = 0 is the MSB, code bit 7) is planes[j][k][n >> 5], column n
+ *     sits at bit (n & 31) of that word.  planes is one allocation of
+ *     8 * K * (N/32) uint32.
+ */
+#ifndef GRINQH_H
+#define GRINQH_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    GRINQH_OK = 0,
+    GRINQH_ERR_NULL = -1,      /* a required pointer is NULL                              */
+    GRINQH_ERR_SHAPE = -2,     /* K % 128, N % 32, T outside 1..4, group != 128, K > max  */
+    GRINQH_ERR_ALIGN = -3,     /* a base pointer is not 16-byte aligned                   */
+    GRINQH_ERR_MIX = -4,       /* sum(counts) != K                                        */
+    GRINQH_ERR_WORKSPACE = -5, /* workspace_bytes smaller than *_workspace_bytes()        */
+    GRINQH_ERR_CUDA = -6       /* a CUDA launch failed; see cudaGetLastError              */
+} grinqh_status;
+
+#define GRINQH_GROUP 128
+#define GRINQH_MAX_T 4
+#define GRINQH_MAX_K 65536      /* assignment runs in one CTA; keys + histogram must fit */
+#define GRINQH_GCNT_STRIDE 16   /* bytes per group in gcnt_ge (entries 0..9 used)        */
+
+/* Static strings, never freed. */
+const char* grinqh_status_string(int status);
+/* major*10000 + minor*100 + patch */
+int grinqh_version(void);
+
+/*
+ * Host helper (Eq. 1: precision distribution P on the simplex).
+ * frac[w] = share of input channels that get w bits, w = 0..8.  Cumulative
+ * rounding from the top width: C_w = floor(K * sum_{v>=w} frac[v] + 0.5),
+ * counts[w] = C_w - C_{w+1}, C_0 forced to K — always sums to K
+ * (reading #3).  Returns GRINQH_ERR_MIX if |sum(frac) - 1| > 1e-6
+ * or any frac < 0.
+ */
+int grinqh_mix_to_counts(int K, const double frac[9], uint32_t counts[9]);
+
+/*
+ * grinqh_pack — offline, once per weight.
+ * Per (group g, column n): lo/hi = min/max of the 128 fp16 values;
+ * s = fp16_rn((float(hi) - float(lo)) / 255), z = lo; if s == 0 all codes are 0,
+ * else q = clamp(rint((float(w) - float(z)) / float(s)), 0, 255), IEEE fp32,
+ * round-half-even, no FMA contraction (reading #8).  Code bit (7-j)
+ * goes to plane j.
+ *   W_f16      dev  [K, N] fp16, read only
+ *   planes     dev  [8][K][N/32] uint32, written
+ *   scales_f16 dev  [K/128][N] fp16, written
+ *   zeros_f16  dev  [K/128][N] fp16, written
+ */
+int grinqh_pack(const void* W_f16, int K, int N, int group,
+                uint32_t* planes, void* scales_f16, void* zeros_f16, void* stream);
+
+/*
+ * grinqh_assign — every decode step, once per input vector
+ * (PAPER.md:61-65 assignment, :271 top-p partition of the live vector).
+ * Per token t: order channels by (|x_tk| descending, k ascending) on the 15
+ * magnitude bits of the fp16 pattern; with C_w = sum_{v>=w} counts[v] the
+ * channel at rank r gets b = max{w : r < C_w} (0 if r >= C_1).
+ *   x_f16       dev   [T, K] fp16
+ *   counts      HOST  [9], counts[w] = rows at width w, sum = K; read during the call
+ *   bits        dev   [T][K] uint8       per-token widths
+ *   bits_union  dev   [K] uint8          max over tokens (the planes actually fetched)
+ *   rows        dev   [K] int32          all channels sorted by (bits_union desc, k asc):
+ *                                        rows[0 : cnt_ge[j+1]] are exactly the rows needing plane j
+ *   cnt_ge      dev   [10] int32         cnt_ge[w] = #{k : bits_union[k] >= w}; cnt_ge[0]=K, cnt_ge[9]=0
+ *   grows       dev   [K] uint8          per 128-row group g, grows[128 g + i] = local index (0..127) of
+ *                                        the i-th row of the group in (bits_union desc, k asc) order
+ *   gcnt_ge     dev   [K/128][16] uint8  gcnt_ge[g][w] = #{k in group g : bits_union[k] >= w}, w = 0..9
+ *                                        (entries 10..15 are zero)
+ *   workspace   dev   >= grinqh_assign_workspace_bytes(T, K) bytes, 16-byte aligned
+ */
+size_t grinqh_assign_workspace_bytes(int T, int K);
+int grinqh_assign(const void* x_f16, int T, int K, const uint32_t counts[9],
+                  uint8_t* bits, uint8_t* bits_union, int32_t* rows, int32_t* cnt_ge,
+                  uint8_t* grows, uint8_t* gcnt_ge,
+                  void* workspace, size_t workspace_bytes, void* stream);
+
+/*
+ * grinqh_vmm — per projection (PAPER.md:85 reconstruction, :51 selective fetch).
+ * Split-K main kernel (CTAs walk the compacted per-group row lists and fetch
+ * only planes j < bits_union[k] of row k) followed by a deterministic
+ * fixed-order second-pass reduce of the split-K partials.  fp32 accumulation.
+ * For T > 1 each token is truncated to its own bits[t][k]; y[t] equals the
+ * T = 1 result of token t alone.
+ *   y          dev  [T, N] fp32, written
+ *   workspace  dev  >= grinqh_vmm_workspace_bytes(T, K, N) bytes, 16-byte aligned
+ * grinqh_vmm_main / grinqh_vmm_reduce are the two halves (main writes the
+ * split-K partials into workspace, reduce sums them into y); grinqh_vmm
+ * enqueues both.
+ */
+size_t grinqh_vmm_workspace_bytes(int T, int K, int N);
+int grinqh_vmm(const void* x_f16, int T, int K, int N, int group,
+               const uint32_t* planes, const void* scales_f16, const void* zeros_f16,
+               const uint8_t* bits, const uint8_t* bits_union,
+               const uint8_t* grows, const uint8_t* gcnt_ge,
+               float* y, void* workspace, size_t workspace_bytes, void* stream);
+int grinqh_vmm_main(const void* x_f16, int T, int K, int N, int group,
+                    const uint32_t* planes, const void* scales_f16, const void* zeros_f16,
+                    const uint8_t* bits, const uint8_t* bits_union,
+                    const uint8_t* grows, const uint8_t* gcnt_ge,
+                    void* workspace, size_t workspace_bytes, void* stream);
+int grinqh_vmm_reduce(int T, int K, int N, float* y,
+                      const void* workspace, size_t workspace_bytes, void* stream);
+
+/*
+ * Host-buffer decode call (the end-to-end entry): copies x from HOST memory to
+ * the device staging buffer x_dev_f16, runs grinqh_assign + grinqh_vmm, and
+ * copies y back to HOST memory, all enqueued on `stream` (cudaMemcpyAsync;
+ * pass pinned host memory for real asynchrony).  The packed weights stay
+ * resident on the device.  The caller synchronises the stream before reading
+ * y_host.
+ *   x_host_f16  HOST [T, K] fp16       y_host  HOST [T, N] fp32
+ *   x_dev_f16   dev  [T, K] fp16 staging, y_dev dev [T, N] fp32 staging
+ *   assign_ws / vmm_ws: device workspaces as above
+ */
+int grinqh_decode_host(const void* x_host_f16, int T, int K, int N, int group,
+                       const uint32_t counts[9],
+                       const uint32_t* planes, const void* scales_f16, const void* zeros_f16,
+                       void* x_dev_f16, uint8_t* bits, uint8_t* bits_union, int32_t* rows, int32_t* cnt_ge,
+                       uint8_t* grows, uint8_t* gcnt_ge,
+                       void* assign_ws, size_t assign_ws_bytes,
+                       float* y_dev, void* vmm_ws, size_t vmm_ws_bytes,
+                       float* y_host, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GRINQH_H */
