@@ -56,7 +56,7 @@ typedef enum {
 
 #define GRINQH_GROUP 128
 #define GRINQH_MAX_T 4
-#define GRINQH_MAX_K 65536      /* assignment runs in one CTA; keys + histogram must fit */
+#define GRINQH_MAX_K 32768      /* assignment runs in one CTA; keys + histogram must fit */
 #define GRINQH_GCNT_STRIDE 16   /* bytes per group in gcnt_ge (entries 0..9 used)        */
 
 /* Static strings, never freed. */

@@ -1,0 +1,190 @@
+"""Thin Python binding over the C ABI in include/grinqh.h (argument marshalling only).
+
+Every step of the path runs inside csrc/libgrinqh.so; torch is used for device memory and streams.
+There is no CPU fallback: if the shared library is missing the import raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "csrc", "libgrinqh.so")
+
+GROUP = 128
+GCNT_STRIDE = 16
+MAX_T = 4
+MAX_K = 32768
+
+if not os.path.exists(LIB_PATH):
+    raise ImportError(
+        f"{LIB_PATH} is missing: build it with `python -m paper_2606_23419_b200.build` "
+        "(or __graft_entry__.build()).  There is no CPU fallback for the GRINQH path.")
+
+_lib = C.CDLL(LIB_PATH)
+
+_vp, _i, _sz = C.c_void_p, C.c_int, C.c_size_t
+_lib.grinqh_status_string.restype = C.c_char_p
+_lib.grinqh_status_string.argtypes = [_i]
+_lib.grinqh_version.restype = _i
+_lib.grinqh_mix_to_counts.restype = _i
+_lib.grinqh_mix_to_counts.argtypes = [_i, _vp, _vp]
+_lib.grinqh_pack.restype = _i
+_lib.grinqh_pack.argtypes = [_vp, _i, _i, _i, _vp, _vp, _vp, _vp]
+_lib.grinqh_assign_workspace_bytes.restype = _sz
+_lib.grinqh_assign_workspace_bytes.argtypes = [_i, _i]
+_lib.grinqh_assign.restype = _i
+_lib.grinqh_assign.argtypes = [_vp, _i, _i, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _sz, _vp]
+_lib.grinqh_vmm_workspace_bytes.restype = _sz
+_lib.grinqh_vmm_workspace_bytes.argtypes = [_i, _i, _i]
+_VMM_COMMON = [_vp, _i, _i, _i, _i, _vp, _vp, _vp, _vp, _vp, _vp, _vp]
+_lib.grinqh_vmm.restype = _i
+_lib.grinqh_vmm.argtypes = _VMM_COMMON + [_vp, _vp, _sz, _vp]
+_lib.grinqh_vmm_main.restype = _i
+_lib.grinqh_vmm_main.argtypes = _VMM_COMMON + [_vp, _sz, _vp]
+_lib.grinqh_vmm_reduce.restype = _i
+_lib.grinqh_vmm_reduce.argtypes = [_i, _i, _i, _vp, _vp, _sz, _vp]
+_lib.grinqh_decode_host.restype = _i
+_lib.grinqh_decode_host.argtypes = [_vp, _i, _i, _i, _i, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp,
+                                    _vp, _sz, _vp, _vp, _sz, _vp, _vp]
+
+EXPORTS = ("grinqh_status_string", "grinqh_version", "grinqh_mix_to_counts", "grinqh_pack",
+           "grinqh_assign_workspace_bytes", "grinqh_assign", "grinqh_vmm_workspace_bytes", "grinqh_vmm",
+           "grinqh_vmm_main", "grinqh_vmm_reduce", "grinqh_decode_host")
+
+
+class GrinqhError(RuntimeError):
+    pass
+
+
+def _check(rc: int, what: str):
+    if rc != 0:
+        raise GrinqhError(f"{what}: {_lib.grinqh_status_string(rc).decode()} ({rc})")
+
+
+def _stream(stream) -> int:
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return stream.cuda_stream
+
+
+def _dev(t: torch.Tensor, dtype, name: str) -> int:
+    if not (t.is_cuda and t.is_contiguous() and t.dtype == dtype):
+        raise GrinqhError(f"{name}: need a contiguous CUDA tensor of {dtype}, got {t.dtype} on {t.device}")
+    return t.data_ptr()
+
+
+def grinqh_version() -> int:
+    return int(_lib.grinqh_version())
+
+
+def grinqh_status_string(rc: int) -> str:
+    return _lib.grinqh_status_string(int(rc)).decode()
+
+
+def grinqh_mix_to_counts(K: int, frac) -> list[int]:
+    f = (C.c_double * 9)(*[float(v) for v in frac])
+    c = (C.c_uint32 * 9)()
+    _check(_lib.grinqh_mix_to_counts(int(K), f, c), "grinqh_mix_to_counts")
+    return [int(v) for v in c]
+
+
+def _counts(counts):
+    return (C.c_uint32 * 9)(*[int(v) for v in counts])
+
+
+class Packed:
+    """Device-resident packed weight: planes [8, K, N/32] int32 (bit patterns), scales/zeros [K/128, N] fp16."""
+
+    def __init__(self, K: int, N: int, device="cuda"):
+        self.K, self.N = K, N
+        self.planes = torch.empty((8, K, N // 32), dtype=torch.int32, device=device)
+        self.scales = torch.empty((K // GROUP, N), dtype=torch.float16, device=device)
+        self.zeros = torch.empty((K // GROUP, N), dtype=torch.float16, device=device)
+
+
+def grinqh_pack(W: torch.Tensor, out: Packed | None = None, stream=None) -> Packed:
+    K, N = W.shape
+    out = out or Packed(K, N, W.device)
+    _check(_lib.grinqh_pack(_dev(W, torch.float16, "W"), K, N, GROUP, out.planes.data_ptr(),
+                            out.scales.data_ptr(), out.zeros.data_ptr(), _stream(stream)), "grinqh_pack")
+    return out
+
+
+class Assignment:
+    """Device buffers written by grinqh_assign for one [T, K] input."""
+
+    def __init__(self, T: int, K: int, device="cuda"):
+        self.T, self.K = T, K
+        self.bits = torch.empty((T, K), dtype=torch.uint8, device=device)
+        self.bits_union = torch.empty((K,), dtype=torch.uint8, device=device)
+        self.rows = torch.empty((K,), dtype=torch.int32, device=device)
+        self.cnt_ge = torch.empty((16,), dtype=torch.int32, device=device)  # 10 used; padded for alignment
+        self.grows = torch.empty((K,), dtype=torch.uint8, device=device)
+        self.gcnt_ge = torch.empty((K // GROUP, GCNT_STRIDE), dtype=torch.uint8, device=device)
+
+
+def grinqh_assign(x: torch.Tensor, counts, out: Assignment | None = None, stream=None) -> Assignment:
+    T, K = x.shape
+    out = out or Assignment(T, K, x.device)
+    _check(_lib.grinqh_assign(_dev(x, torch.float16, "x"), T, K, _counts(counts), out.bits.data_ptr(),
+                              out.bits_union.data_ptr(), out.rows.data_ptr(), out.cnt_ge.data_ptr(),
+                              out.grows.data_ptr(), out.gcnt_ge.data_ptr(), None, 0, _stream(stream)),
+           "grinqh_assign")
+    return out
+
+
+def grinqh_vmm_workspace_bytes(T: int, K: int, N: int) -> int:
+    return int(_lib.grinqh_vmm_workspace_bytes(T, K, N))
+
+
+def _vmm_common(x, w: Packed, a: Assignment):
+    T, K = x.shape
+    return [_dev(x, torch.float16, "x"), T, K, w.N, GROUP, w.planes.data_ptr(), w.scales.data_ptr(),
+            w.zeros.data_ptr(), a.bits.data_ptr(), a.bits_union.data_ptr(), a.grows.data_ptr(),
+            a.gcnt_ge.data_ptr()]
+
+
+def _ws(T, K, N, workspace, device):
+    need = grinqh_vmm_workspace_bytes(T, K, N)
+    if workspace is None:
+        workspace = torch.empty((max(need, 16),), dtype=torch.uint8, device=device)
+    return workspace, workspace.numel() * workspace.element_size()
+
+
+def grinqh_vmm(x: torch.Tensor, w: Packed, a: Assignment, y: torch.Tensor | None = None,
+               workspace: torch.Tensor | None = None, stream=None) -> torch.Tensor:
+    T, K = x.shape
+    if y is None:
+        y = torch.empty((T, w.N), dtype=torch.float32, device=x.device)
+    workspace, nbytes = _ws(T, K, w.N, workspace, x.device)
+    _check(_lib.grinqh_vmm(*_vmm_common(x, w, a), _dev(y, torch.float32, "y"), workspace.data_ptr(), nbytes,
+                           _stream(stream)), "grinqh_vmm")
+    return y
+
+
+def grinqh_vmm_main(x, w: Packed, a: Assignment, workspace: torch.Tensor, stream=None):
+    _check(_lib.grinqh_vmm_main(*_vmm_common(x, w, a), workspace.data_ptr(),
+                                workspace.numel() * workspace.element_size(), _stream(stream)), "grinqh_vmm_main")
+
+
+def grinqh_vmm_reduce(T: int, K: int, N: int, y: torch.Tensor, workspace: torch.Tensor, stream=None):
+    _check(_lib.grinqh_vmm_reduce(T, K, N, _dev(y, torch.float32, "y"), workspace.data_ptr(),
+                                  workspace.numel() * workspace.element_size(), _stream(stream)),
+           "grinqh_vmm_reduce")
+
+
+def grinqh_decode_host(x_host: torch.Tensor, counts, w: Packed, a: Assignment, x_dev: torch.Tensor,
+                       y_dev: torch.Tensor, workspace: torch.Tensor, y_host: torch.Tensor, stream=None):
+    """HOST x [T, K] fp16 (pinned) -> HOST y [T, N] fp32 (pinned); weights stay on the device.  Enqueue only."""
+    T, K = x_host.shape
+    if x_host.is_cuda or y_host.is_cuda:
+        raise GrinqhError("grinqh_decode_host takes HOST x and y")
+    _check(_lib.grinqh_decode_host(
+        x_host.data_ptr(), T, K, w.N, GROUP, _counts(counts), w.planes.data_ptr(), w.scales.data_ptr(),
+        w.zeros.data_ptr(), x_dev.data_ptr(), a.bits.data_ptr(), a.bits_union.data_ptr(), a.rows.data_ptr(),
+        a.cnt_ge.data_ptr(), a.grows.data_ptr(), a.gcnt_ge.data_ptr(), None, 0, y_dev.data_ptr(),
+        workspace.data_ptr(), workspace.numel() * workspace.element_size(), y_host.data_ptr(),
+        _stream(stream)), "grinqh_decode_host")

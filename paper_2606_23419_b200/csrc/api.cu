@@ -1,0 +1,68 @@
+// api.cu — host-side entry points of the C ABI that launch no kernel of their own.
+#include <math.h>
+
+#include "common.cuh"
+
+extern "C" const char* grinqh_status_string(int status) {
+    switch (status) {
+        case GRINQH_OK: return "ok";
+        case GRINQH_ERR_NULL: return "null pointer";
+        case GRINQH_ERR_SHAPE: return "unsupported shape (need K % 128 == 0, N % 32 == 0, 1 <= T <= 4, group == 128, K <= 32768 for assign)";
+        case GRINQH_ERR_ALIGN: return "pointer not 16-byte aligned";
+        case GRINQH_ERR_MIX: return "level mix does not sum to K (or fractions do not sum to 1)";
+        case GRINQH_ERR_WORKSPACE: return "workspace too small";
+        case GRINQH_ERR_CUDA: return "CUDA launch failed";
+        default: return "unknown status";
+    }
+}
+
+extern "C" int grinqh_version(void) { return 100; /* 0.1.0 */ }
+
+// PAPER.md:262-266 (Eq. 1): precision distribution P -> integer row counts; reading #3.
+extern "C" int grinqh_mix_to_counts(int K, const double frac[9], uint32_t counts[9]) {
+    if (!frac || !counts) return GRINQH_ERR_NULL;
+    if (K <= 0) return GRINQH_ERR_SHAPE;
+    double sum = 0.0;
+    for (int w = 0; w < 9; ++w) {
+        if (!(frac[w] >= 0.0)) return GRINQH_ERR_MIX;
+        sum += frac[w];
+    }
+    if (fabs(sum - 1.0) > 1e-6) return GRINQH_ERR_MIX;
+    long long C[10];
+    C[9] = 0;
+    double F = 0.0;
+    for (int w = 8; w >= 1; --w) {
+        F += frac[w];
+        long long c = (long long)floor(F * (double)K + 0.5);
+        if (c < C[w + 1]) c = C[w + 1];
+        if (c > K) c = K;
+        C[w] = c;
+    }
+    C[0] = K;
+    for (int w = 0; w < 9; ++w) counts[w] = (uint32_t)(C[w] - C[w + 1]);
+    return GRINQH_OK;
+}
+
+extern "C" int grinqh_decode_host(const void* x_host_f16, int T, int K, int N, int group, const uint32_t counts[9],
+                                  const uint32_t* planes, const void* scales_f16, const void* zeros_f16,
+                                  void* x_dev_f16, uint8_t* bits, uint8_t* bits_union, int32_t* rows,
+                                  int32_t* cnt_ge, uint8_t* grows, uint8_t* gcnt_ge, void* assign_ws,
+                                  size_t assign_ws_bytes, float* y_dev, void* vmm_ws, size_t vmm_ws_bytes,
+                                  float* y_host, void* stream) {
+    if (!x_host_f16 || !x_dev_f16 || !y_dev || !y_host) return GRINQH_ERR_NULL;
+    if (T < 1 || T > GRINQH_MAX_T || K <= 0 || N <= 0 || K % GQ_G || N % 32 || group != GQ_G || K > GQ_MAX_K)
+        return GRINQH_ERR_SHAPE;
+    if (vmm_ws_bytes < grinqh_vmm_workspace_bytes(T, K, N)) return GRINQH_ERR_WORKSPACE;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (cudaMemcpyAsync(x_dev_f16, x_host_f16, (size_t)T * K * 2, cudaMemcpyHostToDevice, st) != cudaSuccess)
+        return GRINQH_ERR_CUDA;
+    int rc = grinqh_assign(x_dev_f16, T, K, counts, bits, bits_union, rows, cnt_ge, grows, gcnt_ge, assign_ws,
+                           assign_ws_bytes, stream);
+    if (rc != GRINQH_OK) return rc;
+    rc = grinqh_vmm(x_dev_f16, T, K, N, group, planes, scales_f16, zeros_f16, bits, bits_union, grows, gcnt_ge,
+                    y_dev, vmm_ws, vmm_ws_bytes, stream);
+    if (rc != GRINQH_OK) return rc;
+    if (cudaMemcpyAsync(y_host, y_dev, (size_t)T * N * 4, cudaMemcpyDeviceToHost, st) != cudaSuccess)
+        return GRINQH_ERR_CUDA;
+    return GRINQH_OK;
+}

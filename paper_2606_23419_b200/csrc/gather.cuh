@@ -1,0 +1,58 @@
+// gather.cuh — plane words -> truncated codes in byte lanes (SIMD-in-register 8x8 bit transpose).
+//
+// A lane holds one 32-bit word per fetched plane of a weight row: W[j] bit p = code bit (7-j) of column p
+// of the lane's 32-column block (the b-bit code is the top b planes).  gather<B> runs
+// the three butterfly stages of an 8x8 bit-matrix transpose on all four byte lanes at once and returns
+// V[r], r = 0..7, with   byte L of V[r] = truncated code (top B bits, low bits 0) of column 8 L + r.
+// Planes j >= B are treated as zero, so stages that would only move zeros fold away at compile time:
+// 48 logic/shift ops for B = 8, 28 for B = 4, about 20 for B = 2 (per 32 weights).
+//
+// Plain C++ on uint32_t so that the same code is unit-tested on the host (tests/test_host_logic.py).
+#pragma once
+#include <stdint.h>
+
+#if defined(__CUDACC__)
+#define GQ_HD __host__ __device__ __forceinline__
+#else
+#define GQ_HD inline
+#endif
+
+namespace gq {
+
+// transpose step on the pair (lo, hi) = (row i, row i+s) of every 8x8 byte-lane block:
+//   lo' = (lo & m) | ((hi & m) << s),   hi' = ((lo >> s) & m) | (hi & ~m),   m = low s bits of each 2s.
+template <int S>
+GQ_HD void tstep(uint32_t& lo, uint32_t& hi) {
+    constexpr uint32_t m = (S == 1) ? 0x55555555u : (S == 2) ? 0x33333333u : 0x0F0F0F0Fu;
+    const uint32_t nlo = (lo & m) | ((hi & m) << S);
+    const uint32_t nhi = ((lo >> S) & m) | (hi & ~m);
+    lo = nlo;
+    hi = nhi;
+}
+
+// W[j], j < B: plane words (W[j] for j >= B is ignored).  V[r]: byte L = code of column 8L + r.
+template <int B>
+GQ_HD void gather(const uint32_t (&W)[8], uint32_t (&V)[8]) {
+    static_assert(B == 2 || B == 4 || B == 8, "gather is instantiated for 2, 4 or 8 planes");
+    // a[i] carries code bit i = plane 7 - i
+#pragma unroll
+    for (int i = 0; i < 8; ++i) V[i] = (7 - i < B) ? W[7 - i] : 0u;
+    tstep<1>(V[6], V[7]);
+    if (B > 2) tstep<1>(V[4], V[5]);
+    if (B > 4) {
+        tstep<1>(V[0], V[1]);
+        tstep<1>(V[2], V[3]);
+    }
+    tstep<2>(V[4], V[6]);
+    tstep<2>(V[5], V[7]);
+    if (B > 4) {
+        tstep<2>(V[0], V[2]);
+        tstep<2>(V[1], V[3]);
+    }
+    tstep<4>(V[0], V[4]);
+    tstep<4>(V[1], V[5]);
+    tstep<4>(V[2], V[6]);
+    tstep<4>(V[3], V[7]);
+}
+
+}  // namespace gq
