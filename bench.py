@@ -1,0 +1,368 @@
+#!/usr/bin/env python
+"""bench.py — GRINQH decode hot path on B200 (contract: see the task prompt / DESIGN.md "Measurement").
+
+Workload (N = 1): BASELINE.json configs[1] — one Llama-3-8B-shaped layer, batch 1, avg 4 bits:
+7 projections (q,k,v,o,gate,up,down), 4 distinct input vectors (q/k/v and gate/up share one).
+A "step" = one pass of the per-step hot path over one layer: 4 x grinqh_assign + 7 x grinqh_vmm
+(main + reduce).  grinqh_pack is offline (once per weight) and reported separately under "pack".
+The timed loop rotates over LAYERS distinct packed layers (> L2) so every step streams from HBM.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--mix 4] [--layers 4]
+
+`--impl reference` times the CPU oracle (kind "oracle") on a bounded column sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "us per decode step of one Llama-3-8B-shaped layer (4 assigns + 7 bit-planar VMMs), batch 1"
+UNIT = "us"
+
+
+def _args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=2000)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--impl", default="native", choices=["native", "reference"])
+    ap.add_argument("--mix", default="4")
+    ap.add_argument("--layers", type=int, default=4, help="distinct packed layers the timed loop rotates over")
+    ap.add_argument("--seed", type=int, default=0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    return ap.parse_args()
+
+
+def _peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def alg_bytes(K, N, T, sum_bits):
+    """Algorithmic bytes of one VMM: fetched planes + fp16 s,z + x + y + lists."""
+    return (N // 8) * sum_bits + 4 * (K // 128) * N + 2 * T * K + 4 * T * N + 5 * K
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons with NVML during the timed region."""
+
+    def __init__(self, index: int):
+        super().__init__(daemon=True)
+        self.index, self.samples, self.reasons, self.max_mhz, self._stop_evt = index, [], set(), None, threading.Event()
+        self.ok = False
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+            self.ok = True
+        except Exception:
+            pass
+
+    def run(self):
+        if not self.ok:
+            return
+        nv = self.nv
+        names = {
+            getattr(nv, "nvmlClocksEventReasonHwSlowdown", 0x8): "hw_slowdown",
+            getattr(nv, "nvmlClocksEventReasonHwThermalSlowdown", 0x40): "hw_thermal_slowdown",
+            getattr(nv, "nvmlClocksEventReasonSwThermalSlowdown", 0x20): "sw_thermal_slowdown",
+            getattr(nv, "nvmlClocksEventReasonSwPowerCap", 0x4): "sw_power_cap",
+        }
+        while not self._stop_evt.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                try:
+                    r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                except Exception:
+                    r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for bit, name in names.items():
+                    if r & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            time.sleep(0.004)
+
+    def stop(self):
+        self._stop_evt.set()
+        self.join(timeout=1.0)
+        s = sorted(self.samples)
+        return {"sm_mhz": (s[len(s) // 2] if s else None), "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(s)}
+
+
+# ------------------------------------------------------------------------------------------ reference arm
+class OracleLayerSample:
+    """CPU oracle on a bounded sample of the layer step: for each of the 7 projections the first
+    `cols_per_proj` output columns (all K rows) + the 4 assignments.  Packing the sample is offline
+    (not timed).  run() returns the seconds one sampled step took; `fraction` scales it to the full layer."""
+
+    def __init__(self, mix_name: str, seed: int, cols_per_proj: int):
+        import oracle
+        from paper_2606_23419_b200 import synth
+        self.oracle, self.synth = oracle, synth
+        self.frac = synth.MIXES[mix_name]
+        self.xs = {name: synth.make_x(1, K, seed + i, "normal")
+                   for i, (name, K) in enumerate(synth.LLAMA3_8B_INPUT_DIMS.items())}
+        self.packed, full_w, samp_w = {}, 0, 0
+        for i, (name, K, N) in enumerate(synth.LLAMA3_8B_LAYER):
+            n = min(N, cols_per_proj)
+            self.packed[name] = oracle.pack(synth.make_weights(K, n, 0.02, seed + 100 + i))
+            full_w += K * N
+            samp_w += K * n
+        self.fraction = samp_w / full_w
+        self.desc = (f"oracle assign x4 + oracle vmm (fp64, 1 thread) on the first {cols_per_proj} output columns of "
+                     f"each of the 7 projections ({samp_w / 1e6:.2f}M of {full_w / 1e6:.1f}M weights), "
+                     f"time scaled by the weight ratio")
+
+    def run(self) -> float:
+        oracle, synth = self.oracle, self.synth
+        t0 = time.perf_counter()
+        assigns = {}
+        for name, K in synth.LLAMA3_8B_INPUT_DIMS.items():
+            assigns[name] = oracle.assign(self.xs[name], oracle.mix_to_counts(K, self.frac))
+        for name, K, N in synth.LLAMA3_8B_LAYER:
+            inp = synth.LLAMA3_8B_INPUTS[name]
+            planes, s, z = self.packed[name]
+            oracle.vmm(self.xs[inp], planes, s, z, assigns[inp]["bits"])
+        return time.perf_counter() - t0
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from paper_2606_23419_b200 import synth
+    # size the per-step sample so that the whole run stays within ~2 minutes (about 25 ns per weight)
+    budget = 120.0 / max(1, args.steps + args.warmup)
+    rows = sum(K for _, K, _ in synth.LLAMA3_8B_LAYER)
+    cols = int(budget / (rows * 32 * 25e-9)) * 32
+    cols = max(32, min(1024, cols))
+    sample = OracleLayerSample(args.mix, args.seed, cols)
+    times = []
+    for i in range(args.warmup + args.steps):
+        t = sample.run()
+        if i >= args.warmup:
+            times.append(t / sample.fraction)
+    us = 1e6 * sum(times) / len(times)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": us, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": us / 1e3, "higher_is_better": False, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "llama3-8b-layer (BASELINE.json configs[1]), batch 1",
+                   "avg_bits": synth.mix_avg_bits(synth.MIXES[args.mix]), "mix": args.mix},
+        "cpu_baseline": {"value": us, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample.desc},
+        "e2e": {"value": us, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+# ------------------------------------------------------------------------------------------ native arm
+def run_native(args):
+    import numpy as np
+    import torch
+
+    from paper_2606_23419_b200 import binding as gq
+    from paper_2606_23419_b200 import synth
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    frac = synth.MIXES[args.mix]
+    avg_bits = synth.mix_avg_bits(frac)
+    L = args.layers
+    T = 1
+    layer = synth.LLAMA3_8B_LAYER
+    in_dims = synth.LLAMA3_8B_INPUT_DIMS
+    counts = {K: gq.grinqh_mix_to_counts(K, frac) for K in set(in_dims.values())}
+
+    # ---- offline: generate + pack L distinct layers (grinqh_pack timed on its own)
+    gen = torch.Generator(device=dev)
+    gen.manual_seed(args.seed + 1000 * rank)
+    packed, pack_ms, pack_bytes = [], 0.0, 0
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    for l in range(L):
+        d = {}
+        for name, K, N in layer:
+            W = (torch.randn((K, N), generator=gen, device=dev, dtype=torch.float32) * 0.02).to(torch.float16)
+            out = gq.Packed(K, N, dev)
+            torch.cuda.synchronize()
+            e0.record()
+            gq.grinqh_pack(W, out)
+            e1.record()
+            torch.cuda.synchronize()
+            pack_ms += e0.elapsed_time(e1)
+            pack_bytes += K * N * 3 + (K // 128) * N * 4
+            d[name] = out
+            del W
+        packed.append(d)
+
+    # ---- per-step inputs: fresh activations per layer copy (N(0,1), 1% channels x20)
+    x_host = [{n: torch.from_numpy(synth.make_x(T, K, args.seed + 10 * l + i + 1000 * rank, "normal")).pin_memory()
+               for i, (n, K) in enumerate(in_dims.items())} for l in range(L)]
+    x_dev = [{n: v.to(dev) for n, v in xl.items()} for xl in x_host]
+    assigns = [{n: gq.Assignment(T, K, dev) for n, K in in_dims.items()} for _ in range(L)]
+    y_dev = [{name: torch.empty((T, N), dtype=torch.float32, device=dev) for name, K, N in layer} for _ in range(L)]
+    y_host = [{name: torch.empty((T, N), dtype=torch.float32).pin_memory() for name, K, N in layer} for _ in range(L)]
+    ws_bytes = max(gq.grinqh_vmm_workspace_bytes(T, K, N) for _, K, N in layer)
+    ws = torch.empty((ws_bytes,), dtype=torch.uint8, device=dev)
+    x_stage = {n: torch.empty((T, K), dtype=torch.float16, device=dev) for n, K in in_dims.items()}
+
+    def step_device(l):
+        for n, K in in_dims.items():
+            gq.grinqh_assign(x_dev[l][n], counts[K], assigns[l][n])
+        for name, K, N in layer:
+            n = synth.LLAMA3_8B_INPUTS[name]
+            gq.grinqh_vmm(x_dev[l][n], packed[l][name], assigns[l][n], y_dev[l][name], ws)
+
+    def step_main_only(l):
+        for name, K, N in layer:
+            n = synth.LLAMA3_8B_INPUTS[name]
+            gq.grinqh_vmm_main(x_dev[l][n], packed[l][name], assigns[l][n], ws)
+
+    def step_host(l):
+        seen = set()
+        for name, K, N in layer:
+            n = synth.LLAMA3_8B_INPUTS[name]
+            gq.grinqh_decode_host(x_host[l][n], counts[K], packed[l][name], assigns[l][n], x_stage[n],
+                                  y_dev[l][name], ws, y_host[l][name], reuse_assignment=(n in seen))
+            seen.add(n)
+
+    stream = torch.cuda.Stream(device=dev)
+    with torch.cuda.stream(stream):
+        for l in range(L):          # eager warm-up (also configures kernel attributes before capture)
+            step_device(l)
+            step_host(l)
+        stream.synchronize()
+
+        def capture(fn):
+            graphs = []
+            for l in range(L):
+                g = torch.cuda.CUDAGraph()
+                with torch.cuda.graph(g, stream=stream):
+                    fn(l)
+                graphs.append(g)
+            return graphs
+
+        g_dev = capture(step_device)
+        g_main = capture(step_main_only)
+        g_host = capture(step_host)
+
+        def barrier():
+            if world > 1:
+                import torch.distributed as dist
+                dist.barrier()
+            torch.cuda.synchronize()
+
+        def timed(graphs, steps, sync_each=False):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            barrier()
+            a.record(stream)
+            for i in range(steps):
+                graphs[i % L].replay()
+                if sync_each:
+                    stream.synchronize()
+            b.record(stream)
+            barrier()
+            return a.elapsed_time(b)
+
+        for i in range(max(args.warmup, 3)):
+            g_dev[i % L].replay()
+        sampler = ClockSampler(local)
+        sampler.start()
+        ms_total = timed(g_dev, args.steps)
+        clocks = sampler.stop()
+        for i in range(3):
+            g_main[i % L].replay()
+        ms_main = timed(g_main, args.steps)
+        for i in range(3):
+            g_host[i % L].replay()
+        ms_host = timed(g_host, args.steps, sync_each=True)
+
+    if world > 1:
+        import torch.distributed as dist
+        t = torch.tensor([ms_total, ms_main, ms_host], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total, ms_main, ms_host = [float(v) for v in t.tolist()]
+
+    # ---- algorithmic bytes of the 7 main-kernel launches of one step (measured widths)
+    step_bytes, plane_bytes = 0, 0
+    per_vmm = []
+    for name, K, N in layer:
+        n = synth.LLAMA3_8B_INPUTS[name]
+        sb = int(assigns[0][n].bits_union.sum().item())
+        b = alg_bytes(K, N, T, sb)
+        step_bytes += b
+        plane_bytes += (N // 8) * sb
+        per_vmm.append({"proj": name, "K": K, "N": N, "alg_bytes": b})
+    peak, peak_src = _peaks()
+    us_step = ms_total * 1e3 / args.steps
+    us_main = ms_main * 1e3 / args.steps
+    us_host = ms_host * 1e3 / args.steps
+    achieved = step_bytes / (us_main * 1e-6) / 1e9  # GB/s over the 7 vmm_main launches of a step
+
+    h2d = sum(T * K * 2 for K in in_dims.values())
+    d2h = sum(T * N * 4 for _, _, N in layer)
+    line = {
+        "metric": METRIC, "value": us_step / world, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": us_step / 1e3, "higher_is_better": False, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": "llama3-8b-layer (BASELINE.json configs[1]): 4096->4096 x2 (q,o), 4096->1024 x2 (k,v), "
+                               "4096->14336 x2 (gate,up), 14336->4096 (down); batch 1; per-step rank assignment",
+                   "avg_bits": avg_bits, "mix": args.mix, "group": 128, "tokens": T,
+                   "l2": f"timed loop rotates over {L} distinct packed layers "
+                         f"({L * sum(K * N for _, K, N in layer) / 1e6:.0f} MB of planes > 126 MB L2); CUDA graph per layer",
+                   "replicas": "replicas only (no data-path collective)" if world > 1 else "single GPU"},
+        "clocks": clocks,
+        "e2e": {"value": us_host / world, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                "how": "grinqh_decode_host per projection (pinned host x in, pinned host y out), stream sync per step"},
+        "gpu_launches": args.steps * (len(in_dims) + 2 * len(layer)),
+        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                     "traffic": None, "kernel": "vmm_main_kernel<1> (7 launches per step)",
+                     "alg_bytes_per_step": step_bytes, "plane_bytes_per_step": plane_bytes,
+                     "us_per_step_main_only": us_main, "peak_source": peak_src},
+        "pack": {"GBps": pack_bytes / (pack_ms * 1e-3) / 1e9, "ms_per_layer": pack_ms / L},
+        "per_vmm": per_vmm,
+    }
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        sample = OracleLayerSample(args.mix, args.seed, 1024)
+        t = min(sample.run() for _ in range(3))
+        line["cpu_baseline"] = {"value": 1e6 * t / sample.fraction, "unit": UNIT, "cores": 1, "kind": "oracle",
+                                "sample": sample.desc}
+    if rank == 0:
+        print(json.dumps(line))
+    if world > 1:
+        import torch.distributed as dist
+        dist.destroy_process_group()
+
+
+def main():
+    args = _args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_native(args)
+
+
+if __name__ == "__main__":
+    main()

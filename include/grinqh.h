@@ -151,7 +151,11 @@ int grinqh_vmm_reduce(int T, int K, int N, float* y,
  *   x_host_f16  HOST [T, K] fp16       y_host  HOST [T, N] fp32
  *   x_dev_f16   dev  [T, K] fp16 staging, y_dev dev [T, N] fp32 staging
  *   assign_ws / vmm_ws: device workspaces as above
+ *   flags       GRINQH_REUSE_ASSIGNMENT: x_dev_f16 and the assignment buffers already hold this x
+ *               (a previous call for a projection that consumes the same input vector — q/k/v, gate/up);
+ *               skip the host->device copy and grinqh_assign.
  */
+#define GRINQH_REUSE_ASSIGNMENT 1
 int grinqh_decode_host(const void* x_host_f16, int T, int K, int N, int group,
                        const uint32_t counts[9],
                        const uint32_t* planes, const void* scales_f16, const void* zeros_f16,
@@ -159,7 +163,7 @@ int grinqh_decode_host(const void* x_host_f16, int T, int K, int N, int group,
                        uint8_t* grows, uint8_t* gcnt_ge,
                        void* assign_ws, size_t assign_ws_bytes,
                        float* y_dev, void* vmm_ws, size_t vmm_ws_bytes,
-                       float* y_host, void* stream);
+                       float* y_host, int flags, void* stream);
 
 #ifdef __cplusplus
 }
