@@ -233,12 +233,12 @@ def run_native(args):
             gq.grinqh_assign(x_dev[l][n], counts[K], assigns[l][n])
         for name, K, N in layer:
             n = synth.LLAMA3_8B_INPUTS[name]
-            gq.grinqh_vmm(x_dev[l][n], packed[l][name], assigns[l][n], y_dev[l][name], ws)
+            gq.grinqh_vmm(packed[l][name], assigns[l][n], y_dev[l][name], ws)
 
     def step_main_only(l):
         for name, K, N in layer:
             n = synth.LLAMA3_8B_INPUTS[name]
-            gq.grinqh_vmm_main(x_dev[l][n], packed[l][name], assigns[l][n], ws)
+            gq.grinqh_vmm_main(packed[l][name], assigns[l][n], ws)
 
     def step_host(l):
         seen = set()

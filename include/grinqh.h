@@ -106,37 +106,38 @@ int grinqh_pack(const void* W_f16, int K, int N, int group,
  *                                        the i-th row of the group in (bits_union desc, k asc) order
  *   gcnt_ge     dev   [K/128][16] uint8  gcnt_ge[g][w] = #{k in group g : bits_union[k] >= w}, w = 0..9
  *                                        (entries 10..15 are zero)
+ *   gsched      dev   [T][K] uint32      the per-group schedule grinqh_vmm walks: entry [t][128 g + i] describes
+ *                                        the i-th row of group g's list, r = grows[128 g + i], k = 128 g + r:
+ *                                          bits 0..7 r | 8..11 bits[t][k] | 12..15 bits_union[k] | 16..31 x[t][k] (fp16 pattern)
+ *                                        a pure re-indexing of the outputs above (bit-exact against the oracle's)
  *   workspace   dev   >= grinqh_assign_workspace_bytes(T, K) bytes, 16-byte aligned
  */
 size_t grinqh_assign_workspace_bytes(int T, int K);
 int grinqh_assign(const void* x_f16, int T, int K, const uint32_t counts[9],
                   uint8_t* bits, uint8_t* bits_union, int32_t* rows, int32_t* cnt_ge,
-                  uint8_t* grows, uint8_t* gcnt_ge,
+                  uint8_t* grows, uint8_t* gcnt_ge, uint32_t* gsched,
                   void* workspace, size_t workspace_bytes, void* stream);
 
 /*
  * grinqh_vmm — per projection (PAPER.md:85 reconstruction, :51 selective fetch).
- * Split-K main kernel (CTAs walk the compacted per-group row lists and fetch
- * only planes j < bits_union[k] of row k) followed by a deterministic
- * fixed-order second-pass reduce of the split-K partials.  fp32 accumulation.
- * For T > 1 each token is truncated to its own bits[t][k]; y[t] equals the
- * T = 1 result of token t alone.
+ * Split-K main kernel (warps walk the per-group schedule and fetch only planes j < bits_union[k] of row k)
+ * followed by a deterministic fixed-order second-pass reduce of the split-K partials.  fp32 accumulation.
+ * For T > 1 each token is truncated to its own bits[t][k]; y[t] equals the T = 1 result of token t alone.
+ * The activations enter through gsched (x values, widths and row order of the assignment).
+ *   gsched, gcnt_ge   dev   as written by grinqh_assign for this [T, K] input
  *   y          dev  [T, N] fp32, written
  *   workspace  dev  >= grinqh_vmm_workspace_bytes(T, K, N) bytes, 16-byte aligned
- * grinqh_vmm_main / grinqh_vmm_reduce are the two halves (main writes the
- * split-K partials into workspace, reduce sums them into y); grinqh_vmm
- * enqueues both.
+ * grinqh_vmm_main / grinqh_vmm_reduce are the two halves (main writes the split-K partials into
+ * workspace, reduce sums them into y); grinqh_vmm enqueues both.
  */
 size_t grinqh_vmm_workspace_bytes(int T, int K, int N);
-int grinqh_vmm(const void* x_f16, int T, int K, int N, int group,
+int grinqh_vmm(int T, int K, int N, int group,
                const uint32_t* planes, const void* scales_f16, const void* zeros_f16,
-               const uint8_t* bits, const uint8_t* bits_union,
-               const uint8_t* grows, const uint8_t* gcnt_ge,
+               const uint32_t* gsched, const uint8_t* gcnt_ge,
                float* y, void* workspace, size_t workspace_bytes, void* stream);
-int grinqh_vmm_main(const void* x_f16, int T, int K, int N, int group,
+int grinqh_vmm_main(int T, int K, int N, int group,
                     const uint32_t* planes, const void* scales_f16, const void* zeros_f16,
-                    const uint8_t* bits, const uint8_t* bits_union,
-                    const uint8_t* grows, const uint8_t* gcnt_ge,
+                    const uint32_t* gsched, const uint8_t* gcnt_ge,
                     void* workspace, size_t workspace_bytes, void* stream);
 int grinqh_vmm_reduce(int T, int K, int N, float* y,
                       const void* workspace, size_t workspace_bytes, void* stream);
@@ -151,7 +152,7 @@ int grinqh_vmm_reduce(int T, int K, int N, float* y,
  *   x_host_f16  HOST [T, K] fp16       y_host  HOST [T, N] fp32
  *   x_dev_f16   dev  [T, K] fp16 staging, y_dev dev [T, N] fp32 staging
  *   assign_ws / vmm_ws: device workspaces as above
- *   flags       GRINQH_REUSE_ASSIGNMENT: x_dev_f16 and the assignment buffers already hold this x
+ *   flags       GRINQH_REUSE_ASSIGNMENT: the assignment buffers already hold this x
  *               (a previous call for a projection that consumes the same input vector — q/k/v, gate/up);
  *               skip the host->device copy and grinqh_assign.
  */
@@ -160,7 +161,7 @@ int grinqh_decode_host(const void* x_host_f16, int T, int K, int N, int group,
                        const uint32_t counts[9],
                        const uint32_t* planes, const void* scales_f16, const void* zeros_f16,
                        void* x_dev_f16, uint8_t* bits, uint8_t* bits_union, int32_t* rows, int32_t* cnt_ge,
-                       uint8_t* grows, uint8_t* gcnt_ge,
+                       uint8_t* grows, uint8_t* gcnt_ge, uint32_t* gsched,
                        void* assign_ws, size_t assign_ws_bytes,
                        float* y_dev, void* vmm_ws, size_t vmm_ws_bytes,
                        float* y_host, int flags, void* stream);

@@ -36,10 +36,10 @@ _lib.grinqh_pack.argtypes = [_vp, _i, _i, _i, _vp, _vp, _vp, _vp]
 _lib.grinqh_assign_workspace_bytes.restype = _sz
 _lib.grinqh_assign_workspace_bytes.argtypes = [_i, _i]
 _lib.grinqh_assign.restype = _i
-_lib.grinqh_assign.argtypes = [_vp, _i, _i, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _sz, _vp]
+_lib.grinqh_assign.argtypes = [_vp, _i, _i, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _sz, _vp]
 _lib.grinqh_vmm_workspace_bytes.restype = _sz
 _lib.grinqh_vmm_workspace_bytes.argtypes = [_i, _i, _i]
-_VMM_COMMON = [_vp, _i, _i, _i, _i, _vp, _vp, _vp, _vp, _vp, _vp, _vp]
+_VMM_COMMON = [_i, _i, _i, _i, _vp, _vp, _vp, _vp, _vp]
 _lib.grinqh_vmm.restype = _i
 _lib.grinqh_vmm.argtypes = _VMM_COMMON + [_vp, _vp, _sz, _vp]
 _lib.grinqh_vmm_main.restype = _i
@@ -48,7 +48,7 @@ _lib.grinqh_vmm_reduce.restype = _i
 _lib.grinqh_vmm_reduce.argtypes = [_i, _i, _i, _vp, _vp, _sz, _vp]
 _lib.grinqh_decode_host.restype = _i
 _lib.grinqh_decode_host.argtypes = [_vp, _i, _i, _i, _i, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp,
-                                    _vp, _sz, _vp, _vp, _sz, _vp, _i, _vp]
+                                    _vp, _vp, _sz, _vp, _vp, _sz, _vp, _i, _vp]
 
 EXPORTS = ("grinqh_status_string", "grinqh_version", "grinqh_mix_to_counts", "grinqh_pack",
            "grinqh_assign_workspace_bytes", "grinqh_assign", "grinqh_vmm_workspace_bytes", "grinqh_vmm",
@@ -124,6 +124,7 @@ class Assignment:
         self.cnt_ge = torch.empty((16,), dtype=torch.int32, device=device)  # 10 used; padded for alignment
         self.grows = torch.empty((K,), dtype=torch.uint8, device=device)
         self.gcnt_ge = torch.empty((K // GROUP, GCNT_STRIDE), dtype=torch.uint8, device=device)
+        self.gsched = torch.empty((T, K), dtype=torch.int32, device=device)  # uint32 bit patterns
 
 
 def grinqh_assign(x: torch.Tensor, counts, out: Assignment | None = None, stream=None) -> Assignment:
@@ -131,7 +132,8 @@ def grinqh_assign(x: torch.Tensor, counts, out: Assignment | None = None, stream
     out = out or Assignment(T, K, x.device)
     _check(_lib.grinqh_assign(_dev(x, torch.float16, "x"), T, K, _counts(counts), out.bits.data_ptr(),
                               out.bits_union.data_ptr(), out.rows.data_ptr(), out.cnt_ge.data_ptr(),
-                              out.grows.data_ptr(), out.gcnt_ge.data_ptr(), None, 0, _stream(stream)),
+                              out.grows.data_ptr(), out.gcnt_ge.data_ptr(), out.gsched.data_ptr(), None, 0,
+                              _stream(stream)),
            "grinqh_assign")
     return out
 
@@ -140,11 +142,11 @@ def grinqh_vmm_workspace_bytes(T: int, K: int, N: int) -> int:
     return int(_lib.grinqh_vmm_workspace_bytes(T, K, N))
 
 
-def _vmm_common(x, w: Packed, a: Assignment):
-    T, K = x.shape
-    return [_dev(x, torch.float16, "x"), T, K, w.N, GROUP, w.planes.data_ptr(), w.scales.data_ptr(),
-            w.zeros.data_ptr(), a.bits.data_ptr(), a.bits_union.data_ptr(), a.grows.data_ptr(),
-            a.gcnt_ge.data_ptr()]
+def _vmm_common(w: Packed, a: Assignment):
+    if a.K != w.K:
+        raise GrinqhError(f"assignment is for K={a.K}, weight has K={w.K}")
+    return [a.T, a.K, w.N, GROUP, w.planes.data_ptr(), w.scales.data_ptr(), w.zeros.data_ptr(),
+            a.gsched.data_ptr(), a.gcnt_ge.data_ptr()]
 
 
 def _ws(T, K, N, workspace, device):
@@ -154,19 +156,21 @@ def _ws(T, K, N, workspace, device):
     return workspace, workspace.numel() * workspace.element_size()
 
 
-def grinqh_vmm(x: torch.Tensor, w: Packed, a: Assignment, y: torch.Tensor | None = None,
+def grinqh_vmm(w: Packed, a: Assignment, y: torch.Tensor | None = None,
                workspace: torch.Tensor | None = None, stream=None) -> torch.Tensor:
-    T, K = x.shape
+    """y [T, N] fp32 = x . W over the planes the assignment `a` (made from x) selects."""
+    T, K = a.T, a.K
+    dev = w.planes.device
     if y is None:
-        y = torch.empty((T, w.N), dtype=torch.float32, device=x.device)
-    workspace, nbytes = _ws(T, K, w.N, workspace, x.device)
-    _check(_lib.grinqh_vmm(*_vmm_common(x, w, a), _dev(y, torch.float32, "y"), workspace.data_ptr(), nbytes,
+        y = torch.empty((T, w.N), dtype=torch.float32, device=dev)
+    workspace, nbytes = _ws(T, K, w.N, workspace, dev)
+    _check(_lib.grinqh_vmm(*_vmm_common(w, a), _dev(y, torch.float32, "y"), workspace.data_ptr(), nbytes,
                            _stream(stream)), "grinqh_vmm")
     return y
 
 
-def grinqh_vmm_main(x, w: Packed, a: Assignment, workspace: torch.Tensor, stream=None):
-    _check(_lib.grinqh_vmm_main(*_vmm_common(x, w, a), workspace.data_ptr(),
+def grinqh_vmm_main(w: Packed, a: Assignment, workspace: torch.Tensor, stream=None):
+    _check(_lib.grinqh_vmm_main(*_vmm_common(w, a), workspace.data_ptr(),
                                 workspace.numel() * workspace.element_size(), _stream(stream)), "grinqh_vmm_main")
 
 
@@ -186,6 +190,6 @@ def grinqh_decode_host(x_host: torch.Tensor, counts, w: Packed, a: Assignment, x
     _check(_lib.grinqh_decode_host(
         x_host.data_ptr(), T, K, w.N, GROUP, _counts(counts), w.planes.data_ptr(), w.scales.data_ptr(),
         w.zeros.data_ptr(), x_dev.data_ptr(), a.bits.data_ptr(), a.bits_union.data_ptr(), a.rows.data_ptr(),
-        a.cnt_ge.data_ptr(), a.grows.data_ptr(), a.gcnt_ge.data_ptr(), None, 0, y_dev.data_ptr(),
+        a.cnt_ge.data_ptr(), a.grows.data_ptr(), a.gcnt_ge.data_ptr(), a.gsched.data_ptr(), None, 0, y_dev.data_ptr(),
         workspace.data_ptr(), workspace.numel() * workspace.element_size(), y_host.data_ptr(),
         1 if reuse_assignment else 0, _stream(stream)), "grinqh_decode_host")

@@ -46,10 +46,10 @@ extern "C" int grinqh_mix_to_counts(int K, const double frac[9], uint32_t counts
 extern "C" int grinqh_decode_host(const void* x_host_f16, int T, int K, int N, int group, const uint32_t counts[9],
                                   const uint32_t* planes, const void* scales_f16, const void* zeros_f16,
                                   void* x_dev_f16, uint8_t* bits, uint8_t* bits_union, int32_t* rows,
-                                  int32_t* cnt_ge, uint8_t* grows, uint8_t* gcnt_ge, void* assign_ws,
-                                  size_t assign_ws_bytes, float* y_dev, void* vmm_ws, size_t vmm_ws_bytes,
+                                  int32_t* cnt_ge, uint8_t* grows, uint8_t* gcnt_ge, uint32_t* gsched,
+                                  void* assign_ws, size_t assign_ws_bytes, float* y_dev, void* vmm_ws, size_t vmm_ws_bytes,
                                   float* y_host, int flags, void* stream) {
-    if (!x_host_f16 || !x_dev_f16 || !y_dev || !y_host) return GRINQH_ERR_NULL;
+    if (!x_host_f16 || !x_dev_f16 || !y_dev || !y_host || !gsched) return GRINQH_ERR_NULL;
     if (T < 1 || T > GRINQH_MAX_T || K <= 0 || N <= 0 || K % GQ_G || N % 32 || group != GQ_G || K > GQ_MAX_K)
         return GRINQH_ERR_SHAPE;
     if (vmm_ws_bytes < grinqh_vmm_workspace_bytes(T, K, N)) return GRINQH_ERR_WORKSPACE;
@@ -58,12 +58,12 @@ extern "C" int grinqh_decode_host(const void* x_host_f16, int T, int K, int N, i
     if (!(flags & GRINQH_REUSE_ASSIGNMENT)) {
         if (cudaMemcpyAsync(x_dev_f16, x_host_f16, (size_t)T * K * 2, cudaMemcpyHostToDevice, st) != cudaSuccess)
             return GRINQH_ERR_CUDA;
-        rc = grinqh_assign(x_dev_f16, T, K, counts, bits, bits_union, rows, cnt_ge, grows, gcnt_ge, assign_ws,
-                           assign_ws_bytes, stream);
+        rc = grinqh_assign(x_dev_f16, T, K, counts, bits, bits_union, rows, cnt_ge, grows, gcnt_ge, gsched,
+                           assign_ws, assign_ws_bytes, stream);
         if (rc != GRINQH_OK) return rc;
     }
-    rc = grinqh_vmm(x_dev_f16, T, K, N, group, planes, scales_f16, zeros_f16, bits, bits_union, grows, gcnt_ge,
-                    y_dev, vmm_ws, vmm_ws_bytes, stream);
+    rc = grinqh_vmm(T, K, N, group, planes, scales_f16, zeros_f16, gsched, gcnt_ge, y_dev, vmm_ws, vmm_ws_bytes,
+                    stream);
     if (rc != GRINQH_OK) return rc;
     if (cudaMemcpyAsync(y_host, y_dev, (size_t)T * N * 4, cudaMemcpyDeviceToHost, st) != cudaSuccess)
         return GRINQH_ERR_CUDA;

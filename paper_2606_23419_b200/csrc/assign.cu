@@ -1,269 +1,331 @@
-// assign.cu — grinqh_assign: |x| ranking -> per-channel bit widths -> compacted row lists.
+// assign.cu — grinqh_assign: |x| ranking -> per-channel bit widths -> compacted row lists (v2).
 // PAPER.md:61-65 (assignment), :271 (top-p partition of the live vector); readings #2-#4.
 //
-// One CTA of 1024 threads.  Per token: a 32768-bin shared-memory histogram (u16 bins, padded so that
-// each thread's 32 bins load conflict-free) of the 15-bit fp16 magnitudes, a block scan to find the (at most 8) histogram bins that contain a cut C_w, and an
-// ordered (index-ascending) count inside those bins so that ties go to the lower index.  No sort.
-// Then the union over tokens, the global (width desc, index asc) list by a 9-way stable partition,
-// and the per-128-row-group lists by warp ballots.
+// One CTA of 1024 threads, no sort.  Per token a two-level radix select on the 15-bit fp16 magnitude:
+//   level 1  256-bin histogram of key >> 7 (8 sub-histograms against atomic contention); one warp scans it
+//            from the top and finds, for each of the (at most 8) cuts C_w, the bin that contains it;
+//   level 2  128-bin histograms of key & 127 restricted to those bins; warp w finds the exact cut key thr_w,
+//            how many of the keys equal to thr_w are still inside (take_w), and whether the cut splits a run
+//            of equal keys.
+// Widths are then b = #{w : key >= thr_w}.  Only if some cut splits a tie run (ties go to the lower index) an
+// ordered count of the equal keys (per 128-row group, then a scan over groups) decides them.
+// Lists: one warp per 128-row group partitions its rows by (width desc, index asc) with ballots -> grows,
+// gcnt_ge, gsched; a scan over the groups' per-width counts places every group's runs in the global `rows`.
 #include "common.cuh"
 
 namespace gq {
 
-constexpr int AT = 1024;       // threads
-constexpr int HIST_TSTRIDE = 80;                 // bytes per thread: 32 u16 bins + 16 B pad (bank spread)
-constexpr int HIST_BYTES = AT * HIST_TSTRIDE;    // 80 KB
-constexpr int SROW = AT + AT / 32;               // padded scratch row: entry tid lives at tid + tid/32
-constexpr int SCRATCH_BYTES = 9 * SROW * 4;      // 38016
-static_assert(SCRATCH_BYTES % 16 == 0 && SCRATCH_BYTES + GQ_MAX_K <= HIST_BYTES, "alias layout");
-__device__ __forceinline__ int sidx(int tid) { return tid + (tid >> 5); }
+constexpr int AT = 1024;  // threads
+constexpr int AWARPS = AT / 32;
+constexpr int NSUB = 8;
+constexpr int MAXG = GQ_MAX_K / GQ_G;  // 256 groups
 
 struct AssignParams {
     int T, K;
     int C[10];  // C[w] = rows with width >= w (C[0] = K, C[9] = 0)
 };
 
-// inclusive block scan of one int per thread (1024 threads); red = 32-int shared scratch
-__device__ __forceinline__ int block_scan_incl(int v, int* red) {
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+__device__ __forceinline__ int warp_incl_scan(int v, int lane) {
 #pragma unroll
     for (int d = 1; d < 32; d <<= 1) {
-        int o = __shfl_up_sync(0xffffffffu, v, d);
+        const int o = __shfl_up_sync(0xffffffffu, v, d);
         if (lane >= d) v += o;
     }
-    if (lane == 31) red[warp] = v;
-    __syncthreads();
-    if (warp == 0) {
-        int w = red[lane];
-#pragma unroll
-        for (int d = 1; d < 32; d <<= 1) {
-            int o = __shfl_up_sync(0xffffffffu, w, d);
-            if (lane >= d) w += o;
-        }
-        red[lane] = w;
-    }
-    __syncthreads();
-    if (warp > 0) v += red[warp - 1];
-    __syncthreads();
     return v;
 }
 
-// rows of `scratch` ([nrows][SROW] ints, entry tid at sidx(tid)) -> exclusive prefix over the AT
-// entries, in place; totals[row] = sum.  Warp `row` scans row `row`; lane l owns entries 32l..32l+31,
-// which sit at 33l + i: conflict-free.
-__device__ __forceinline__ void scan_rows_excl(int* scratch, int nrows, int* totals) {
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    if (warp < nrows) {
-        int* row = scratch + warp * SROW + lane * 33;
-        int s = 0;
-#pragma unroll 8
-        for (int i = 0; i < 32; ++i) s += row[i];
-        int incl = s;
+// tab[g][col], g < groups: exclusive prefix over g, in place; returns the total to lane 31's caller via *tot.
+// One warp per column; lane l owns groups 8l..8l+7.
+__device__ __forceinline__ void scan_groups(uint16_t (*tab)[10], int col, int groups, int lane, int* tot) {
+    int v[8], s = 0;
 #pragma unroll
-        for (int d = 1; d < 32; d <<= 1) {
-            int o = __shfl_up_sync(0xffffffffu, incl, d);
-            if (lane >= d) incl += o;
-        }
-        int run = incl - s;
-#pragma unroll 8
-        for (int i = 0; i < 32; ++i) {
-            int v = row[i];
-            row[i] = run;
-            run += v;
-        }
-        if (lane == 31) totals[warp] = incl;
+    for (int i = 0; i < 8; ++i) {
+        const int g = 8 * lane + i;
+        v[i] = (g < groups) ? tab[g][col] : 0;
+        s += v[i];
     }
+    const int incl = warp_incl_scan(s, lane);
+    int run = incl - s;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        const int g = 8 * lane + i;
+        if (g < groups) tab[g][col] = (uint16_t)run;
+        run += v[i];
+    }
+    if (lane == 31) *tot = incl;
 }
 
 __global__ void __launch_bounds__(AT, 1)
 assign_kernel(const uint16_t* __restrict__ x, AssignParams p, uint8_t* __restrict__ bits,
               uint8_t* __restrict__ bits_union, int32_t* __restrict__ rows, int32_t* __restrict__ cnt_ge,
-              uint8_t* __restrict__ grows, uint8_t* __restrict__ gcnt_ge) {
+              uint8_t* __restrict__ grows, uint8_t* __restrict__ gcnt_ge, uint32_t* __restrict__ gsched) {
     extern __shared__ __align__(16) uint8_t smem[];
-    uint8_t* hist = smem;                                                // 80 KB, u16 bins, padded per thread
-    int* scratch = reinterpret_cast<int*>(smem);                         // aliases hist: [9][SROW] ints
-    uint8_t* tokbits = smem + SCRATCH_BYTES;                             // aliases hist beyond scratch: K bytes
-    uint16_t* keys = reinterpret_cast<uint16_t*>(smem + HIST_BYTES);     // K u16
-    uint8_t* ubits = smem + HIST_BYTES + GQ_MAX_K * 2;                   // K u8
-    __shared__ int red[32];
-    __shared__ int s_cutbin[9], s_take[9], s_tot[9];
+    uint16_t* keys = reinterpret_cast<uint16_t*>(smem);  // K u16 (current token); later aliased by glist (K u8)
+    uint8_t* glist = smem;
+    uint8_t* ubits = smem + (size_t)p.K * 2;             // K u8, union of the token widths
+    __shared__ uint32_t hist1[NSUB][256];
+    __shared__ uint32_t hist2[8][128];
+    __shared__ uint16_t tab[MAXG][10];
+    __shared__ int s_B[9], s_above[9], s_thr[9], s_take[9], s_split[9], s_tot[10];
+    __shared__ int s_anysplit;
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int K = p.K;
-    const int chunk = (K + AT - 1) / AT;
-    const int k0 = min(K, tid * chunk), k1 = min(K, k0 + chunk);
+    const int K = p.K, groups = K / GQ_G;
+    const uint32_t lt_mask = (1u << lane) - 1u;
 
     for (int t = 0; t < p.T; ++t) {
-        // A. clear histogram
+        // ---- P0: clear, keys, level-1 histogram
+        for (int i = tid; i < NSUB * 256; i += AT) (&hist1[0][0])[i] = 0;
+        (&hist2[0][0])[tid] = 0;
+        if (tid < 9) {
+            s_B[tid] = -1;
+            s_above[tid] = 0;
+            s_thr[tid] = 0x8000;  // above every key: no channel reaches this width
+            s_take[tid] = 0;
+            s_split[tid] = 0;
+        }
+        if (tid == 0) s_anysplit = 0;
+        __syncthreads();
         {
-            uint4* h4 = reinterpret_cast<uint4*>(hist);
-            for (int i = tid; i < HIST_BYTES / 16; i += AT) h4[i] = make_uint4(0, 0, 0, 0);
-            if (tid < 9) {
-                s_cutbin[tid] = 0x8000;  // above every key: no channel reaches this width
-                s_take[tid] = 0;
+            const uint32_t* x2 = reinterpret_cast<const uint32_t*>(x + (size_t)t * K);
+            uint32_t* h = hist1[warp & (NSUB - 1)];
+            for (int i = tid; i < K / 2; i += AT) {
+                const uint32_t v = x2[i] & 0x7FFF7FFFu;
+                reinterpret_cast<uint32_t*>(keys)[i] = v;
+                atomicAdd(&h[(v & 0xFFFFu) >> 7], 1u);
+                atomicAdd(&h[v >> 23], 1u);
             }
         }
         __syncthreads();
-        // B. keys + histogram
-        for (int k = tid; k < K; k += AT) {
-            uint16_t m = x[(size_t)t * K + k] & 0x7FFFu;
-            keys[k] = m;
-            // u16 bin inside a 32-bit word; a bin never exceeds K <= 32768, so no carry into its neighbour
-            atomicAdd(reinterpret_cast<uint32_t*>(hist + (m >> 5) * HIST_TSTRIDE + ((m & 31) >> 1) * 4),
-                      1u << ((m & 1) * 16));
-        }
-        __syncthreads();
-        // C. per-thread sum of its 32 bins, block scan -> number of keys in higher bins
-        uint32_t loc[32];
-        {
-            const uint4* h4 = reinterpret_cast<const uint4*>(hist + tid * HIST_TSTRIDE);
+        // ---- P1: warp 0 scans the 256 bins from the top and locates the bin of every cut
+        if (warp == 0) {
+            int h[8], s = 0;
 #pragma unroll
-            for (int i = 0; i < 4; ++i) {
-                const uint4 v = h4[i];
-                loc[8 * i + 0] = v.x & 0xFFFFu; loc[8 * i + 1] = v.x >> 16;
-                loc[8 * i + 2] = v.y & 0xFFFFu; loc[8 * i + 3] = v.y >> 16;
-                loc[8 * i + 4] = v.z & 0xFFFFu; loc[8 * i + 5] = v.z >> 16;
-                loc[8 * i + 6] = v.w & 0xFFFFu; loc[8 * i + 7] = v.w >> 16;
+            for (int i = 0; i < 8; ++i) {
+                const int bin = 255 - 8 * lane - i;
+                int c = 0;
+#pragma unroll
+                for (int u = 0; u < NSUB; ++u) c += (int)hist1[u][bin];
+                h[i] = c;
+                s += c;
             }
-        }
-        int tsum = 0;
+            const int above = warp_incl_scan(s, lane) - s;
 #pragma unroll
-        for (int i = 0; i < 32; ++i) tsum += (int)loc[i];
-        const int incl = block_scan_incl(tsum, red);
-        const int above = K - incl;  // keys strictly above this thread's bins
-        // D. locate cut bins
-        bool mine = false;
+            for (int w = 1; w <= 8; ++w) {
+                const int Cw = p.C[w];
+                if (Cw > 0 && above < Cw && Cw <= above + s) {
+                    int run = above;
+                    bool done = false;
 #pragma unroll
-        for (int w = 1; w <= 8; ++w) mine |= (above < p.C[w]) && (p.C[w] <= above + tsum);
-        if (mine) {
-            int G = above;
-#pragma unroll
-            for (int i = 31; i >= 0; --i) {
-                const int h = (int)loc[i];
-                if (h > 0) {
-#pragma unroll
-                    for (int w = 1; w <= 8; ++w)
-                        if (G < p.C[w] && p.C[w] <= G + h) {
-                            s_cutbin[w] = tid * 32 + i;
-                            s_take[w] = p.C[w] - G;
+                    for (int i = 0; i < 8; ++i) {
+                        if (!done && Cw <= run + h[i]) {
+                            s_B[w] = 255 - 8 * lane - i;
+                            s_above[w] = run;
+                            done = true;
                         }
+                        run += h[i];
+                    }
                 }
-                G += h;
             }
         }
-        __syncthreads();  // hist no longer needed: scratch / tokbits alias it from here on
-        int cutbin[9], take[9];
+        __syncthreads();
+        // ---- P2: level-2 histograms inside the cut bins (cuts that share a bin share histogram `slot`)
+        int B[9], slot[9];
+#pragma unroll
+        for (int w = 1; w <= 8; ++w) B[w] = s_B[w];
 #pragma unroll
         for (int w = 1; w <= 8; ++w) {
-            cutbin[w] = s_cutbin[w];
-            take[w] = s_take[w];
+            slot[w] = w;
+#pragma unroll
+            for (int v = w - 1; v >= 1; --v)
+                if (B[v] == B[w]) slot[w] = v;
         }
-        // E. ordered tie counts inside the cut bins
-        {
-            int cnt[9];
+        for (int i = tid; i < K; i += AT) {
+            const int m = keys[i];
+            const int top = m >> 7;
 #pragma unroll
-            for (int w = 1; w <= 8; ++w) cnt[w] = 0;
-            for (int k = k0; k < k1; ++k) {
-                const int m = keys[k];
-#pragma unroll
-                for (int w = 1; w <= 8; ++w) cnt[w] += (m == cutbin[w]);
-            }
-#pragma unroll
-            for (int w = 1; w <= 8; ++w) scratch[(w - 1) * SROW + sidx(tid)] = cnt[w];
+            for (int w = 1; w <= 8; ++w)
+                if (top == B[w] && slot[w] == w) atomicAdd(&hist2[w - 1][m & 127], 1u);
         }
         __syncthreads();
-        scan_rows_excl(scratch, 8, s_tot);
-        __syncthreads();
-        // G. widths
-        {
-            int run[9];
+        // ---- P3: warp w-1 finds the exact cut key of cut w
+        if (warp < 8) {
+            const int w = warp + 1;
+            int Bw = -1, sl = 1, ab = 0;
 #pragma unroll
-            for (int w = 1; w <= 8; ++w) run[w] = scratch[(w - 1) * SROW + sidx(tid)];
-            for (int k = k0; k < k1; ++k) {
-                const int m = keys[k];
-                int b = 0;
+            for (int v = 1; v <= 8; ++v)
+                if (v == w) { Bw = B[v]; sl = slot[v]; }
+            ab = s_above[w];
+            if (Bw >= 0) {
+                const int need = p.C[w] - ab;  // 1 <= need <= keys in bin Bw
+                int h[4], s = 0;
 #pragma unroll
-                for (int w = 1; w <= 8; ++w) {
-                    const bool eq = (m == cutbin[w]);
-                    b += (m > cutbin[w]) || (eq && run[w] < take[w]);
-                    run[w] += eq;
+                for (int i = 0; i < 4; ++i) {
+                    h[i] = (int)hist2[sl - 1][127 - 4 * lane - i];
+                    s += h[i];
                 }
-                tokbits[k] = (uint8_t)b;
-                ubits[k] = (t == 0) ? (uint8_t)b : max(ubits[k], (uint8_t)b);
+                const int above = warp_incl_scan(s, lane) - s;
+                if (above < need && need <= above + s) {
+                    int run = above;
+                    bool done = false;
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) {
+                        if (!done && need <= run + h[i]) {
+                            s_thr[w] = (Bw << 7) | (127 - 4 * lane - i);
+                            s_take[w] = need - run;
+                            if (need - run < h[i]) {
+                                s_split[w] = 1;
+                                s_anysplit = 1;
+                            }
+                            done = true;
+                        }
+                        run += h[i];
+                    }
+                }
             }
         }
         __syncthreads();
-        {
-            const uint4* src = reinterpret_cast<const uint4*>(tokbits);
-            uint4* dst = reinterpret_cast<uint4*>(bits + (size_t)t * K);
-            for (int i = tid; i < K / 16; i += AT) dst[i] = src[i];
+        int thr[9], take[9], split[9];
+#pragma unroll
+        for (int w = 1; w <= 8; ++w) {
+            thr[w] = s_thr[w];
+            take[w] = s_take[w];
+            split[w] = s_split[w];
+        }
+        const bool anysplit = s_anysplit != 0;
+        if (anysplit) {
+            // ---- a cut splits a run of equal keys: ordered (index-ascending) count of the equal keys
+            for (int g = warp; g < groups; g += AWARPS) {
+                const uint2 kv = *reinterpret_cast<const uint2*>(keys + g * GQ_G + 4 * lane);
+                const int m[4] = {(int)(kv.x & 0xFFFF), (int)(kv.x >> 16), (int)(kv.y & 0xFFFF), (int)(kv.y >> 16)};
+#pragma unroll
+                for (int w = 1; w <= 8; ++w)
+                    if (split[w]) {
+                        int c = 0;
+#pragma unroll
+                        for (int i = 0; i < 4; ++i) c += (m[i] == thr[w]);
+                        c = __reduce_add_sync(0xffffffffu, c);
+                        if (lane == 0) tab[g][w] = (uint16_t)c;
+                    }
+            }
+            __syncthreads();
+            if (warp < 8 && split[warp + 1]) {
+                int dummy;
+                scan_groups(tab, warp + 1, groups, lane, &dummy);
+            }
+            __syncthreads();
+        }
+        // ---- P4: widths of this token
+        for (int g = warp; g < groups; g += AWARPS) {
+            const uint2 kv = *reinterpret_cast<const uint2*>(keys + g * GQ_G + 4 * lane);
+            const int m[4] = {(int)(kv.x & 0xFFFF), (int)(kv.x >> 16), (int)(kv.y & 0xFFFF), (int)(kv.y >> 16)};
+            int b[4] = {0, 0, 0, 0};
+#pragma unroll
+            for (int w = 1; w <= 8; ++w) {
+                if (!split[w]) {
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) b[i] += (m[i] >= thr[w]);
+                } else {
+                    bool eq[4];
+                    int below = tab[g][w];  // equal keys in earlier groups
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) {
+                        eq[i] = (m[i] == thr[w]);
+                        below += __popc(__ballot_sync(0xffffffffu, eq[i]) & lt_mask);
+                    }
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) {
+                        b[i] += (m[i] > thr[w]) || (eq[i] && below < take[w]);
+                        below += eq[i];
+                    }
+                }
+            }
+            const uint32_t packed = (uint32_t)b[0] | ((uint32_t)b[1] << 8) | ((uint32_t)b[2] << 16) | ((uint32_t)b[3] << 24);
+            *reinterpret_cast<uint32_t*>(bits + (size_t)t * K + g * GQ_G + 4 * lane) = packed;
+            uint32_t* u = reinterpret_cast<uint32_t*>(ubits + g * GQ_G + 4 * lane);
+            *u = (t == 0) ? packed : __vmaxu4(*u, packed);
         }
         __syncthreads();
     }
 
-    // H. union out
-    {
-        const uint4* src = reinterpret_cast<const uint4*>(ubits);
-        uint4* dst = reinterpret_cast<uint4*>(bits_union);
-        for (int i = tid; i < K / 16; i += AT) dst[i] = src[i];
-    }
-    // I. global list: stable 9-way partition, width descending, index ascending
-    {
-        int cnt[9];
+    // ---- P5: per-group lists (keys are dead: glist aliases them)
+    __shared__ __align__(16) uint8_t gcs[MAXG][GQ_GCNT];
+    for (int g = warp; g < groups; g += AWARPS) {
+        const uint32_t bu4 = *reinterpret_cast<const uint32_t*>(ubits + g * GQ_G + 4 * lane);
+        *reinterpret_cast<uint32_t*>(bits_union + g * GQ_G + 4 * lane) = bu4;
+        int bu[4], pos[4];
 #pragma unroll
-        for (int w = 0; w < 9; ++w) cnt[w] = 0;
-        for (int k = k0; k < k1; ++k) {
-            const int b = ubits[k];
+        for (int i = 0; i < 4; ++i) bu[i] = (bu4 >> (8 * i)) & 0xFF;
+        int base = 0, myge = 0, myn = 0;
 #pragma unroll
-            for (int w = 0; w < 9; ++w) cnt[w] += (b == w);
-        }
+        for (int c = 8; c >= 0; --c) {
+            int lower = base, n = 0;
 #pragma unroll
-        for (int w = 0; w < 9; ++w) scratch[w * SROW + sidx(tid)] = cnt[w];
-    }
-    __syncthreads();
-    scan_rows_excl(scratch, 9, s_tot);
-    __syncthreads();
-    {
-        int base[9], acc = 0;
-#pragma unroll
-        for (int w = 8; w >= 0; --w) {
-            base[w] = acc + scratch[w * SROW + sidx(tid)];
-            acc += s_tot[w];
-        }
-        for (int k = k0; k < k1; ++k) {
-            const int b = ubits[k];
-            int pos = 0;
-#pragma unroll
-            for (int w = 0; w < 9; ++w)
-                if (b == w) {
-                    pos = base[w];
-                    base[w]++;
-                }
-            rows[pos] = k;
-        }
-        if (tid < 10) {
-            int c = 0;
-            for (int w = 8; w >= tid; --w) c += s_tot[w];
-            cnt_ge[tid] = (tid == 9) ? 0 : c;
-        }
-    }
-    // J. per-group lists: one warp per 128-row group
-    for (int g = warp; g < K / GQ_G; g += AT / 32) {
-        int b[4];
-#pragma unroll
-        for (int r = 0; r < 4; ++r) b[r] = ubits[g * GQ_G + lane + 32 * r];
-        int base = 0, myge = 0;
-#pragma unroll
-        for (int w = 8; w >= 0; --w) {
-#pragma unroll
-            for (int r = 0; r < 4; ++r) {
-                const uint32_t m = __ballot_sync(0xffffffffu, b[r] == w);
-                if (b[r] == w) grows[g * GQ_G + base + __popc(m & ((1u << lane) - 1u))] = (uint8_t)(lane + 32 * r);
-                base += __popc(m);
+            for (int i = 0; i < 4; ++i) {
+                const uint32_t m = __ballot_sync(0xffffffffu, bu[i] == c);
+                lower += __popc(m & lt_mask);
+                n += __popc(m);
             }
-            if (lane == w) myge = base;
+#pragma unroll
+            for (int i = 0; i < 4; ++i)
+                if (bu[i] == c) pos[i] = lower++;
+            base += n;
+            if (lane == c) {
+                myge = base;
+                myn = n;
+            }
         }
-        if (lane < GQ_GCNT) gcnt_ge[g * GQ_GCNT + lane] = (uint8_t)(lane <= 8 ? myge : 0);
+        if (lane < GQ_GCNT) {
+            const uint8_t v = (uint8_t)(lane <= 8 ? myge : 0);
+            gcnt_ge[g * GQ_GCNT + lane] = v;
+            gcs[g][lane] = v;
+        }
+        if (lane < 9) tab[g][lane] = (uint16_t)myn;
+#pragma unroll
+        for (int i = 0; i < 4; ++i) glist[g * GQ_G + pos[i]] = (uint8_t)(4 * lane + i);
+        for (int t = 0; t < p.T; ++t) {
+            const uint32_t bt4 = *reinterpret_cast<const uint32_t*>(bits + (size_t)t * K + g * GQ_G + 4 * lane);
+            const uint2 xv = *reinterpret_cast<const uint2*>(x + (size_t)t * K + g * GQ_G + 4 * lane);
+            const uint32_t xs[4] = {xv.x & 0xFFFFu, xv.x >> 16, xv.y & 0xFFFFu, xv.y >> 16};
+#pragma unroll
+            for (int i = 0; i < 4; ++i)
+                gsched[(size_t)t * K + g * GQ_G + pos[i]] = (uint32_t)(4 * lane + i) | (((bt4 >> (8 * i)) & 0xFFu) << 8) |
+                                                            ((uint32_t)bu[i] << 12) | (xs[i] << 16);
+        }
+        __syncwarp();
+        *reinterpret_cast<uint32_t*>(grows + g * GQ_G + 4 * lane) =
+            *reinterpret_cast<const uint32_t*>(glist + g * GQ_G + 4 * lane);
+    }
+    __syncthreads();
+    // ---- P6: where each group's run of every width starts in the global list
+    if (warp < 9) scan_groups(tab, warp, groups, lane, &s_tot[warp]);
+    __syncthreads();
+    // ---- P7: global list (width desc, index asc) and cnt_ge
+    int cbase[9];
+    {
+        int acc = 0;
+#pragma unroll
+        for (int c = 8; c >= 0; --c) {
+            cbase[c] = acc;
+            acc += s_tot[c];
+        }
+    }
+    if (tid < 10) cnt_ge[tid] = (tid == 9) ? 0 : cbase[tid] + s_tot[tid];
+    for (int g = warp; g < groups; g += AWARPS) {
+        const uint4 cv = *reinterpret_cast<const uint4*>(gcs[g]);
+        const int cge[10] = {(int)(cv.x & 0xFF), (int)((cv.x >> 8) & 0xFF), (int)((cv.x >> 16) & 0xFF), (int)(cv.x >> 24),
+                             (int)(cv.y & 0xFF), (int)((cv.y >> 8) & 0xFF), (int)((cv.y >> 16) & 0xFF), (int)(cv.y >> 24),
+                             (int)(cv.z & 0xFF), 0};
+        const uint32_t l4 = *reinterpret_cast<const uint32_t*>(glist + g * GQ_G + 4 * lane);
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const int pp = 4 * lane + i;
+            int dst = 0;
+#pragma unroll
+            for (int c = 0; c <= 8; ++c)
+                if (pp < cge[c] && pp >= cge[c + 1]) dst = cbase[c] + (int)tab[g][c] + (pp - cge[c + 1]);
+            rows[dst] = g * GQ_G + (int)((l4 >> (8 * i)) & 0xFF);
+        }
     }
 }
 
@@ -277,13 +339,14 @@ extern "C" size_t grinqh_assign_workspace_bytes(int T, int K) {
 
 extern "C" int grinqh_assign(const void* x_f16, int T, int K, const uint32_t counts[9], uint8_t* bits,
                              uint8_t* bits_union, int32_t* rows, int32_t* cnt_ge, uint8_t* grows, uint8_t* gcnt_ge,
-                             void* workspace, size_t workspace_bytes, void* stream) {
+                             uint32_t* gsched, void* workspace, size_t workspace_bytes, void* stream) {
     (void)workspace;
     (void)workspace_bytes;
-    if (!x_f16 || !counts || !bits || !bits_union || !rows || !cnt_ge || !grows || !gcnt_ge) return GRINQH_ERR_NULL;
+    if (!x_f16 || !counts || !bits || !bits_union || !rows || !cnt_ge || !grows || !gcnt_ge || !gsched)
+        return GRINQH_ERR_NULL;
     if (T < 1 || T > GRINQH_MAX_T || K <= 0 || K % GQ_G || K > GQ_MAX_K) return GRINQH_ERR_SHAPE;
     if (((uintptr_t)x_f16 | (uintptr_t)bits | (uintptr_t)bits_union | (uintptr_t)rows | (uintptr_t)cnt_ge |
-         (uintptr_t)grows | (uintptr_t)gcnt_ge) & 15)
+         (uintptr_t)grows | (uintptr_t)gcnt_ge | (uintptr_t)gsched) & 15)
         return GRINQH_ERR_ALIGN;
     unsigned long long total = 0;
     for (int w = 0; w < 9; ++w) total += counts[w];
@@ -293,15 +356,15 @@ extern "C" int grinqh_assign(const void* x_f16, int T, int K, const uint32_t cou
     p.K = K;
     p.C[9] = 0;
     for (int w = 8; w >= 0; --w) p.C[w] = p.C[w + 1] + (int)counts[w];
-    const size_t smem = (size_t)gq::HIST_BYTES + (size_t)GQ_MAX_K * 2 + (size_t)GQ_MAX_K;
+    const size_t smem = (size_t)K * 3;
     static bool configured = false;
     if (!configured) {
-        if (cudaFuncSetAttribute(gq::assign_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) !=
+        if (cudaFuncSetAttribute(gq::assign_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, GQ_MAX_K * 3) !=
             cudaSuccess)
             return GRINQH_ERR_CUDA;
         configured = true;
     }
     gq::assign_kernel<<<1, gq::AT, smem, (cudaStream_t)stream>>>((const uint16_t*)x_f16, p, bits, bits_union, rows,
-                                                                cnt_ge, grows, gcnt_ge);
+                                                                cnt_ge, grows, gcnt_ge, gsched);
     return cudaGetLastError() == cudaSuccess ? GRINQH_OK : GRINQH_ERR_CUDA;
 }

@@ -19,6 +19,8 @@
 // CTA epilogue: the 8 warps' accumulators are added in fixed order and written as one split-K partial
 // part[sx][t][n]; vmm_reduce sums the Sx partials in fixed order.  Everything is deterministic.
 #include "common.cuh"
+#include <type_traits>
+
 #include "gather.cuh"
 
 namespace gq {
@@ -34,13 +36,12 @@ constexpr int CTAS_PER_SM = 2;
 template <int T>
 struct Cfg {
     static constexpr int RING = (T == 1) ? 8 : 4;
-    // per-warp shared memory: ring | yacc[T] | meta[128] u32 | x[T][128] u16 | tb[T][128] u8
+    // per-warp shared memory: ring | yacc[T] | item[128] {entry, row byte offset} | tok[T-1][128] entries
     static constexpr int RING_OFF = 0;
     static constexpr int YACC_OFF = RING * SLOT_BYTES;
-    static constexpr int META_OFF = YACC_OFF + T * YSLOT * 4;
-    static constexpr int X_OFF = META_OFF + 512;
-    static constexpr int TB_OFF = X_OFF + T * 256;
-    static constexpr int WARP_BYTES = TB_OFF + T * 128;
+    static constexpr int ITEM_OFF = YACC_OFF + T * YSLOT * 4;
+    static constexpr int TOK_OFF = ITEM_OFF + 1024;
+    static constexpr int WARP_BYTES = TOK_OFF + (T - 1) * 512;
     static constexpr int SMEM = VW * WARP_BYTES;
     static_assert(WARP_BYTES % 16 == 0, "warp regions stay 16-byte aligned");
 };
@@ -103,39 +104,20 @@ __device__ __forceinline__ void accumulate_row(const uint32_t (&V)[8], uint16_t 
     }
 }
 
-// plane words of one row (ring slot) -> truncated codes V; b is warp-uniform
-__device__ __forceinline__ void expand_row(const uint32_t* slot, int lane, int b, uint32_t (&V)[8]) {
-    uint32_t Wd[8];
-    if (b == 8) {
-#pragma unroll
-        for (int j = 0; j < 8; ++j) Wd[j] = slot[j * 32 + lane];
-        gather<8>(Wd, V);
-    } else if (b == 4) {
-#pragma unroll
-        for (int j = 0; j < 4; ++j) Wd[j] = slot[j * 32 + lane];
-        gather<4>(Wd, V);
-    } else if (b == 2) {
-#pragma unroll
-        for (int j = 0; j < 2; ++j) Wd[j] = slot[j * 32 + lane];
-        gather<2>(Wd, V);
-    } else {  // any other width: stale slot words beyond the row's planes are masked off
-#pragma unroll
-        for (int j = 0; j < 8; ++j) Wd[j] = (j < b) ? slot[j * 32 + lane] : 0u;
-        gather<8>(Wd, V);
-    }
-}
-
 // A16: every plane row is 16-byte aligned (N % 128 == 0) -> LDGSTS.128, 4 planes per instruction;
 // otherwise each lane copies its own word of every plane with 4-byte cp.async.
+//
+// gsched[t][g*128 + p] (written by grinqh_assign) is position p of group g's list for token t:
+//   bits 0..7 local row r | 8..11 b_t (token's width) | 12..15 b (union width = planes fetched) | 16..31 x_t[r] fp16
 template <int T, bool A16>
 __global__ void __launch_bounds__(VTHREADS, (T <= 2) ? CTAS_PER_SM : 1)
-vmm_main_kernel(const uint16_t* __restrict__ x, int K, int N, int Q, int ipw,
-                const uint32_t* __restrict__ planes, const __half* __restrict__ scales,
-                const __half* __restrict__ zeros, const uint8_t* __restrict__ bits,
-                const uint8_t* __restrict__ grows, const uint8_t* __restrict__ gcnt_ge,
+vmm_main_kernel(int K, int N, int Q, int ipw, const uint32_t* __restrict__ planes,
+                const __half* __restrict__ scales, const __half* __restrict__ zeros,
+                const uint32_t* __restrict__ gsched, const uint8_t* __restrict__ gcnt_ge,
                 float* __restrict__ part) {
     using C = Cfg<T>;
     constexpr int RING = C::RING;
+    constexpr uint32_t RING_MASK = RING * SLOT_BYTES - 1;
     extern __shared__ __align__(16) uint8_t smem[];
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -143,22 +125,23 @@ vmm_main_kernel(const uint16_t* __restrict__ x, int K, int N, int Q, int ipw,
     const int words = N >> 5;
     const int word = tile * 32 + lane;
     const bool active = word < words;
-    const size_t pstride = (size_t)K * words;
-    const int groups = K / GQ_G;
-    const int I = groups * Q;
+    const uint32_t rowbytes = (uint32_t)words * 4u;
+    const size_t pbytes = (size_t)K * rowbytes;  // one plane
+    const int I = (K / GQ_G) * Q;
 
     uint8_t* wbase = smem + warp * C::WARP_BYTES;
-    const uint32_t* ring = reinterpret_cast<const uint32_t*>(wbase + C::RING_OFF);
+    const uint8_t* ring = wbase + C::RING_OFF;
     float* yacc = reinterpret_cast<float*>(wbase + C::YACC_OFF);
-    uint32_t* s_meta = reinterpret_cast<uint32_t*>(wbase + C::META_OFF);
-    uint16_t* s_x = reinterpret_cast<uint16_t*>(wbase + C::X_OFF);
-    uint8_t* s_tb = wbase + C::TB_OFF;
+    uint2* s_item = reinterpret_cast<uint2*>(wbase + C::ITEM_OFF);
+    uint32_t* s_tok = reinterpret_cast<uint32_t*>(wbase + C::TOK_OFF);
     const uint32_t ring_s = (uint32_t)__cvta_generic_to_shared(wbase + C::RING_OFF);
 
-    // per-lane copy geometry
+    // per-lane copy geometry: lane copies chunk `seg` (16 B) of plane pj (and pj + 4); pjx = 99 disables the lane
     const int pj = lane >> 3, seg = lane & 7;
     const bool chunk_ok = A16 ? (tile * 32 + seg * 4 < words) : active;
-    const uint32_t* lane_src = A16 ? planes + (size_t)pj * pstride + tile * 32 + seg * 4 : planes + word;
+    const int pjx = chunk_ok ? (A16 ? pj : 0) : 99;
+    const uint8_t* lane_src = reinterpret_cast<const uint8_t*>(planes) +
+                              (A16 ? (size_t)pj * pbytes + (size_t)(tile * 32 + seg * 4) * 4 : (size_t)word * 4);
     const uint32_t lane_dst = A16 ? ring_s + pj * 128 + seg * 16 : ring_s + lane * 4;
 
     const int ws = sx * VW + warp;
@@ -169,45 +152,38 @@ vmm_main_kernel(const uint16_t* __restrict__ x, int K, int N, int Q, int ipw,
     for (int it = it0; it < it1; ++it) {
         const int g = it / Q, q = it - g * Q;
         __syncwarp();
-        // ---- meta: positions 4l..4l+3 of the group's list
-        const uint32_t lst = *reinterpret_cast<const uint32_t*>(grows + g * GQ_G + 4 * lane);
+        // ---- item prologue: lane l stages item rows l, l+32, ... and the warp reduces X, Phi
         const uint4 cv = *reinterpret_cast<const uint4*>(gcnt_ge + g * GQ_GCNT);
-#pragma unroll
-        for (int t = 0; t < T; ++t) {
-            *reinterpret_cast<uint2*>(s_x + t * GQ_G + 4 * lane) =
-                *reinterpret_cast<const uint2*>(x + (size_t)t * K + g * GQ_G + 4 * lane);
-            if (T > 1)
-                *reinterpret_cast<uint32_t*>(s_tb + t * GQ_G + 4 * lane) =
-                    *reinterpret_cast<const uint32_t*>(bits + (size_t)t * K + g * GQ_G + 4 * lane);
-        }
-        __syncwarp();
-        const int nnz = (cv.x >> 8) & 0xFF;  // cnt[1]
+        auto rows_ge = [&](uint32_t c) -> int {  // rows of this item among the first c list positions
+            return ((int)c > q) ? ((int)c - q + Q - 1) / Q : 0;
+        };
+        const int n_rows = rows_ge((cv.x >> 8) & 0xFF);
         float X[T], Phi[T];
 #pragma unroll
         for (int t = 0; t < T; ++t) X[t] = Phi[t] = 0.f;
-        uint32_t mt[4];
 #pragma unroll
-        for (int i = 0; i < 4; ++i) {
-            const int p = 4 * lane + i;
-            const int r = (lst >> (8 * i)) & 0xFF;
-            int b = 0;  // b = #{w in 1..8 : p < cnt[w]}
-            b += (p < (int)((cv.x >> 8) & 0xFF)) + (p < (int)((cv.x >> 16) & 0xFF)) + (p < (int)(cv.x >> 24));
-            b += (p < (int)(cv.y & 0xFF)) + (p < (int)((cv.y >> 8) & 0xFF)) + (p < (int)((cv.y >> 16) & 0xFF)) +
-                 (p < (int)(cv.y >> 24));
-            b += (p < (int)(cv.z & 0xFF));
-            mt[i] = (uint32_t)r | ((uint32_t)b << 8) | ((uint32_t)s_x[r] << 16);
-            const bool mine = (p < nnz) && (p >= q) && ((p - q) % Q == 0);
+        for (int jj = 0; jj < 4; ++jj) {
+            const int i = lane + 32 * jj;
+            if (i < n_rows) {
+                const int p = g * GQ_G + q + i * Q;
+                const uint32_t e0 = gsched[p];
+                s_item[i] = make_uint2(e0, (e0 & 0xFFu) * rowbytes);
 #pragma unroll
-            for (int t = 0; t < T; ++t) {
-                const int bt = (T == 1) ? b : (int)s_tb[t * GQ_G + r];
-                if (mine && bt > 0) {
-                    const float xf = __half2float(__ushort_as_half(s_x[t * GQ_G + r]));
-                    X[t] += xf;
-                    Phi[t] = fmaf(xf, (float)(0x80 >> bt), Phi[t]);  // phi_b = 2^(7-b), phi_8 = 0
+                for (int t = 0; t < T; ++t) {
+                    uint32_t e = e0;
+                    if (t > 0) {
+                        e = gsched[(size_t)t * K + p];
+                        s_tok[(t - 1) * GQ_G + i] = e;
+                    }
+                    const int bt = (e >> 8) & 15;
+                    if (bt > 0) {
+                        const float xf = __half2float(__ushort_as_half((uint16_t)(e >> 16)));
+                        X[t] += xf;
+                        Phi[t] = fmaf(xf, (float)(0x80 >> bt), Phi[t]);  // phi_b = 2^(7-b), phi_8 = 0
+                    }
                 }
             }
         }
-        *reinterpret_cast<uint4*>(s_meta + 4 * lane) = make_uint4(mt[0], mt[1], mt[2], mt[3]);
 #pragma unroll
         for (int t = 0; t < T; ++t)
 #pragma unroll
@@ -216,24 +192,7 @@ vmm_main_kernel(const uint16_t* __restrict__ x, int K, int N, int Q, int ipw,
                 Phi[t] += __shfl_xor_sync(0xffffffffu, Phi[t], d);
             }
         __syncwarp();
-
-        const int n_rows = (nnz > q) ? (nnz - q + Q - 1) / Q : 0;
-        const uint32_t* item_src = lane_src + (size_t)g * GQ_G * words;
-
-        auto issue = [&](int i) {
-            const uint32_t m = s_meta[q + i * Q];
-            const int r = m & 0xFF, b = (m >> 8) & 0xFF;
-            const uint32_t* src = item_src + (uint32_t)(r * words);
-            const uint32_t dst = lane_dst + (i % RING) * SLOT_BYTES;
-            if (A16) {
-                if (chunk_ok && pj < b) cp_async16(dst, src);
-                if (b > 4 && chunk_ok && pj + 4 < b) cp_async16(dst + 512, src + 4 * pstride);
-            } else {
-#pragma unroll
-                for (int j = 0; j < 8; ++j)
-                    if (chunk_ok && j < b) cp_async4(dst + j * 128, src + j * pstride);
-            }
-        };
+        const uint8_t* item_src = lane_src + (size_t)g * GQ_G * rowbytes;
 
         float acc[T][32];
 #pragma unroll
@@ -241,35 +200,94 @@ vmm_main_kernel(const uint16_t* __restrict__ x, int K, int N, int Q, int ipw,
 #pragma unroll
             for (int c = 0; c < 32; ++c) acc[t][c] = 0.f;
 
+        // copy of item row ii into ring slot at byte offset `so`; HI = the row may have more than 4 planes
+        auto issue = [&](int ii, uint32_t so, auto hi_tag) {
+            constexpr bool HI = decltype(hi_tag)::value;
+            const uint2 m = s_item[ii];
+            const int b = (m.x >> 12) & 15;
+            const uint8_t* src = item_src + m.y;
+            const uint32_t dst = lane_dst + so;
+            if (A16) {
+                if (pjx < b) cp_async16(dst, src);
+                if (HI && pjx + 4 < b) cp_async16(dst + 512, src + 4 * pbytes);
+            } else {
+#pragma unroll
+                for (int j = 0; j < (HI ? 8 : 4); ++j)
+                    if (pjx + j < b) cp_async4(dst + j * 128, src + j * pbytes);
+            }
+        };
+        using HiT = std::integral_constant<bool, true>;
+        using LoT = std::integral_constant<bool, false>;
+
+        uint32_t so = 0;  // ring byte offset of the row being consumed
 #pragma unroll
         for (int i = 0; i < RING - 1; ++i) {
-            if (i < n_rows) issue(i);
+            if (i < n_rows) issue(i, i * SLOT_BYTES, HiT{});
             cp_async_commit();
         }
-        for (int i = 0; i < n_rows; ++i) {
-            cp_async_wait<RING - 2>();
-            __syncwarp();
-            if (i + RING - 1 < n_rows) issue(i + RING - 1);
-            cp_async_commit();
-            const uint32_t m = s_meta[q + i * Q];
-            const int b = (m >> 8) & 0xFF;
-            uint32_t V[8];
-            expand_row(ring + (i % RING) * (SLOT_BYTES / 4), lane, b, V);
-            if (T == 1) {
-                accumulate_row(V, (uint16_t)(m >> 16), acc[0]);
-            } else {
-                const int r = m & 0xFF;
+
+        // rows [i0, i1) of the item, all of width B (B = 0: any width, read from the schedule)
+        auto run = [&](auto b_tag, auto hi_tag, int i0, int i1) {
+            constexpr int B = decltype(b_tag)::value;
+            for (int i = i0; i < i1; ++i) {
+                cp_async_wait<RING - 2>();
+                __syncwarp();
+                if (i + RING - 1 < n_rows) issue(i + RING - 1, (so - SLOT_BYTES) & RING_MASK, hi_tag);
+                cp_async_commit();
+                const uint32_t m = s_item[i].x;
+                const uint32_t* slot = reinterpret_cast<const uint32_t*>(ring + so) + lane;
+                so = (so + SLOT_BYTES) & RING_MASK;
+                uint32_t Wd[8], V[8];
+                if (B == 8) {
 #pragma unroll
-                for (int t = 0; t < T; ++t) {
-                    const int bt = s_tb[t * GQ_G + r];  // this token's own width (<= b, the union)
-                    if (bt == 0) continue;              // warp-uniform
-                    const uint32_t mask = 0x01010101u * ((0xFF00u >> bt) & 0xFFu);
-                    uint32_t Vm[8];
+                    for (int j = 0; j < 8; ++j) Wd[j] = slot[j * 32];
+                    gather<8>(Wd, V);
+                } else if (B == 4) {
 #pragma unroll
-                    for (int j = 0; j < 8; ++j) Vm[j] = V[j] & mask;
-                    accumulate_row(Vm, s_x[t * GQ_G + r], acc[t]);
+                    for (int j = 0; j < 4; ++j) Wd[j] = slot[j * 32];
+                    gather<4>(Wd, V);
+                } else if (B == 2) {
+#pragma unroll
+                    for (int j = 0; j < 2; ++j) Wd[j] = slot[j * 32];
+                    gather<2>(Wd, V);
+                } else {  // stale slot words beyond the row's planes are masked off
+                    const int b = (m >> 12) & 15;
+#pragma unroll
+                    for (int j = 0; j < 8; ++j) Wd[j] = (j < b) ? slot[j * 32] : 0u;
+                    gather<8>(Wd, V);
+                }
+                if (T == 1) {
+                    accumulate_row(V, (uint16_t)(m >> 16), acc[0]);
+                } else {
+                    const int b = (m >> 12) & 15;
+#pragma unroll
+                    for (int t = 0; t < T; ++t) {
+                        const uint32_t e = (t == 0) ? m : s_tok[(t - 1) * GQ_G + i];
+                        const int bt = (e >> 8) & 15;  // this token's own width (<= b, the union)
+                        if (bt == 0) continue;         // warp-uniform
+                        if (bt == b) {
+                            accumulate_row(V, (uint16_t)(e >> 16), acc[t]);
+                        } else {
+                            const uint32_t mask = 0x01010101u * ((0xFF00u >> bt) & 0xFFu);
+                            uint32_t Vm[8];
+#pragma unroll
+                            for (int j = 0; j < 8; ++j) Vm[j] = V[j] & mask;
+                            accumulate_row(Vm, (uint16_t)(e >> 16), acc[t]);
+                        }
+                    }
                 }
             }
+        };
+        {
+            using std::integral_constant;
+            const int r8 = rows_ge(cv.z & 0xFF), r5 = rows_ge((cv.y >> 8) & 0xFF), r4 = rows_ge(cv.y & 0xFF);
+            const int r3 = rows_ge(cv.x >> 24), r2 = rows_ge((cv.x >> 16) & 0xFF);
+            run(integral_constant<int, 8>{}, HiT{}, 0, r8);
+            run(integral_constant<int, 0>{}, HiT{}, r8, r5);
+            run(integral_constant<int, 4>{}, LoT{}, r5, r4);
+            run(integral_constant<int, 0>{}, LoT{}, r4, r3);
+            run(integral_constant<int, 2>{}, LoT{}, r3, r2);
+            run(integral_constant<int, 0>{}, LoT{}, r2, n_rows);
         }
         cp_async_wait<0>();
 
@@ -359,9 +377,9 @@ vmm_reduce_kernel(const float* __restrict__ part, int S, int T, int N, float* __
 }
 
 template <int T, bool A16>
-static int launch_main_impl(const void* x, int K, int N, const VmmPlan& pl, const uint32_t* planes, const void* scales,
-                            const void* zeros, const uint8_t* bits, const uint8_t* grows, const uint8_t* gcnt_ge,
-                            float* part, cudaStream_t st) {
+static int launch_main_impl(int K, int N, const VmmPlan& pl, const uint32_t* planes, const void* scales,
+                            const void* zeros, const uint32_t* gsched, const uint8_t* gcnt_ge, float* part,
+                            cudaStream_t st) {
     constexpr int smem = Cfg<T>::SMEM;
     static bool configured = false;
     if (!configured) {
@@ -371,19 +389,17 @@ static int launch_main_impl(const void* x, int K, int N, const VmmPlan& pl, cons
         configured = true;
     }
     dim3 grid(pl.col_tiles, pl.Sx);
-    vmm_main_kernel<T, A16><<<grid, VTHREADS, smem, st>>>((const uint16_t*)x, K, N, pl.Q, pl.ipw, planes,
-                                                          (const __half*)scales, (const __half*)zeros, bits, grows,
-                                                          gcnt_ge, part);
+    vmm_main_kernel<T, A16><<<grid, VTHREADS, smem, st>>>(K, N, pl.Q, pl.ipw, planes, (const __half*)scales,
+                                                          (const __half*)zeros, gsched, gcnt_ge, part);
     return cudaGetLastError() == cudaSuccess ? GRINQH_OK : GRINQH_ERR_CUDA;
 }
 
 template <int T>
-static int launch_main(const void* x, int K, int N, const VmmPlan& pl, const uint32_t* planes, const void* scales,
-                       const void* zeros, const uint8_t* bits, const uint8_t* grows, const uint8_t* gcnt_ge,
-                       float* part, cudaStream_t st) {
-    if (N % 128 == 0)
-        return launch_main_impl<T, true>(x, K, N, pl, planes, scales, zeros, bits, grows, gcnt_ge, part, st);
-    return launch_main_impl<T, false>(x, K, N, pl, planes, scales, zeros, bits, grows, gcnt_ge, part, st);
+static int launch_main(int K, int N, const VmmPlan& pl, const uint32_t* planes, const void* scales,
+                       const void* zeros, const uint32_t* gsched, const uint8_t* gcnt_ge, float* part,
+                       cudaStream_t st) {
+    if (N % 128 == 0) return launch_main_impl<T, true>(K, N, pl, planes, scales, zeros, gsched, gcnt_ge, part, st);
+    return launch_main_impl<T, false>(K, N, pl, planes, scales, zeros, gsched, gcnt_ge, part, st);
 }
 
 static int check_vmm_args(int T, int K, int N, int group) {
@@ -399,26 +415,24 @@ extern "C" size_t grinqh_vmm_workspace_bytes(int T, int K, int N) {
     return (size_t)pl.Sx * T * N * sizeof(float);
 }
 
-extern "C" int grinqh_vmm_main(const void* x_f16, int T, int K, int N, int group, const uint32_t* planes,
-                               const void* scales_f16, const void* zeros_f16, const uint8_t* bits,
-                               const uint8_t* bits_union, const uint8_t* grows, const uint8_t* gcnt_ge,
+extern "C" int grinqh_vmm_main(int T, int K, int N, int group, const uint32_t* planes, const void* scales_f16,
+                               const void* zeros_f16, const uint32_t* gsched, const uint8_t* gcnt_ge,
                                void* workspace, size_t workspace_bytes, void* stream) {
-    if (!x_f16 || !planes || !scales_f16 || !zeros_f16 || !bits || !bits_union || !grows || !gcnt_ge || !workspace)
-        return GRINQH_ERR_NULL;
+    if (!planes || !scales_f16 || !zeros_f16 || !gsched || !gcnt_ge || !workspace) return GRINQH_ERR_NULL;
     int rc = gq::check_vmm_args(T, K, N, group);
     if (rc != GRINQH_OK) return rc;
-    if (((uintptr_t)x_f16 | (uintptr_t)planes | (uintptr_t)scales_f16 | (uintptr_t)zeros_f16 | (uintptr_t)bits |
-         (uintptr_t)grows | (uintptr_t)gcnt_ge | (uintptr_t)workspace) & 15)
+    if (((uintptr_t)planes | (uintptr_t)scales_f16 | (uintptr_t)zeros_f16 | (uintptr_t)gsched |
+         (uintptr_t)gcnt_ge | (uintptr_t)workspace) & 15)
         return GRINQH_ERR_ALIGN;
     if (workspace_bytes < grinqh_vmm_workspace_bytes(T, K, N)) return GRINQH_ERR_WORKSPACE;
     const gq::VmmPlan pl = gq::vmm_plan(T, K, N);
     cudaStream_t st = (cudaStream_t)stream;
     float* part = (float*)workspace;
     switch (T) {
-        case 1: return gq::launch_main<1>(x_f16, K, N, pl, planes, scales_f16, zeros_f16, bits, grows, gcnt_ge, part, st);
-        case 2: return gq::launch_main<2>(x_f16, K, N, pl, planes, scales_f16, zeros_f16, bits, grows, gcnt_ge, part, st);
-        case 3: return gq::launch_main<3>(x_f16, K, N, pl, planes, scales_f16, zeros_f16, bits, grows, gcnt_ge, part, st);
-        default: return gq::launch_main<4>(x_f16, K, N, pl, planes, scales_f16, zeros_f16, bits, grows, gcnt_ge, part, st);
+        case 1: return gq::launch_main<1>(K, N, pl, planes, scales_f16, zeros_f16, gsched, gcnt_ge, part, st);
+        case 2: return gq::launch_main<2>(K, N, pl, planes, scales_f16, zeros_f16, gsched, gcnt_ge, part, st);
+        case 3: return gq::launch_main<3>(K, N, pl, planes, scales_f16, zeros_f16, gsched, gcnt_ge, part, st);
+        default: return gq::launch_main<4>(K, N, pl, planes, scales_f16, zeros_f16, gsched, gcnt_ge, part, st);
     }
 }
 
@@ -435,14 +449,13 @@ extern "C" int grinqh_vmm_reduce(int T, int K, int N, float* y, const void* work
     return cudaGetLastError() == cudaSuccess ? GRINQH_OK : GRINQH_ERR_CUDA;
 }
 
-extern "C" int grinqh_vmm(const void* x_f16, int T, int K, int N, int group, const uint32_t* planes,
-                          const void* scales_f16, const void* zeros_f16, const uint8_t* bits,
-                          const uint8_t* bits_union, const uint8_t* grows, const uint8_t* gcnt_ge, float* y,
+extern "C" int grinqh_vmm(int T, int K, int N, int group, const uint32_t* planes, const void* scales_f16,
+                          const void* zeros_f16, const uint32_t* gsched, const uint8_t* gcnt_ge, float* y,
                           void* workspace, size_t workspace_bytes, void* stream) {
     if (!y) return GRINQH_ERR_NULL;
     if ((uintptr_t)y & 15) return GRINQH_ERR_ALIGN;
-    int rc = grinqh_vmm_main(x_f16, T, K, N, group, planes, scales_f16, zeros_f16, bits, bits_union, grows, gcnt_ge,
-                             workspace, workspace_bytes, stream);
+    int rc = grinqh_vmm_main(T, K, N, group, planes, scales_f16, zeros_f16, gsched, gcnt_ge, workspace,
+                             workspace_bytes, stream);
     if (rc != GRINQH_OK) return rc;
     return grinqh_vmm_reduce(T, K, N, y, workspace, workspace_bytes, stream);
 }

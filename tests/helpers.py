@@ -33,3 +33,18 @@ def rel_l2(a, b):
     d = np.linalg.norm(a - b)
     n = np.linalg.norm(b)
     return d / n if n > 0 else d
+
+
+def expected_gsched(ref: dict, x: np.ndarray, G: int = 128) -> np.ndarray:
+    """include/grinqh.h `gsched`: a pure re-indexing of the oracle's assignment outputs and of x.
+    entry [t][G g + i]: r = grows[G g + i], k = G g + r ->
+    r | bits[t][k] << 8 | bits_union[k] << 12 | fp16 pattern of x[t][k] << 16."""
+    xb = np.ascontiguousarray(x).view(np.uint16).reshape(ref["bits"].shape).astype(np.uint32)
+    T, K = xb.shape
+    r = ref["grows"].astype(np.uint32)
+    k = (np.arange(K, dtype=np.uint32) // G) * G + r
+    out = np.empty((T, K), dtype=np.uint32)
+    for t in range(T):
+        out[t] = r | (ref["bits"][t][k].astype(np.uint32) << 8) | (ref["bits_union"][k].astype(np.uint32) << 12) \
+            | (xb[t][k] << 16)
+    return out

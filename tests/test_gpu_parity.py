@@ -6,7 +6,7 @@ import torch
 
 import oracle
 from paper_2606_23419_b200 import synth
-from tests.helpers import rel_l2
+from tests.helpers import expected_gsched, rel_l2
 
 pytestmark = pytest.mark.gpu
 TOL = 1e-3
@@ -36,7 +36,8 @@ def _check_pack(ref, out):
     assert np.array_equal(out.zeros.cpu().numpy().view(np.uint16), z.view(np.uint16))
 
 
-def _check_assign(ref, a):
+def _check_assign(ref, a, x):
+    assert np.array_equal(a.gsched.cpu().numpy().view(np.uint32), expected_gsched(ref, x))
     assert np.array_equal(a.bits.cpu().numpy(), ref["bits"])
     assert np.array_equal(a.bits_union.cpu().numpy(), ref["bits_union"])
     assert np.array_equal(a.rows.cpu().numpy(), ref["rows"])
@@ -79,7 +80,7 @@ def test_assign_bit_exact(gq, T, K, mix, dist, seed):
     ref = oracle.assign(x, counts)
     a = gq.grinqh_assign(_dev(x), counts)
     torch.cuda.synchronize()
-    _check_assign(ref, a)
+    _check_assign(ref, a, x)
 
 
 def test_assign_ties_and_degenerate_inputs(gq):
@@ -102,7 +103,7 @@ def test_assign_ties_and_degenerate_inputs(gq):
             ref = oracle.assign(x, counts)
             a = gq.grinqh_assign(_dev(x), counts)
             torch.cuda.synchronize()
-            _check_assign(ref, a)
+            _check_assign(ref, a, x)
 
 
 def _run_vmm(gq, W, x, frac):
@@ -114,7 +115,7 @@ def _run_vmm(gq, W, x, frac):
     xd = _dev(x)
     w = gq.grinqh_pack(_dev(W))
     a = gq.grinqh_assign(xd, counts)
-    y = gq.grinqh_vmm(xd, w, a)
+    y = gq.grinqh_vmm(w, a)
     torch.cuda.synchronize()
     return y.cpu().numpy(), y_ref
 
@@ -171,15 +172,15 @@ def test_vmm_one_hot_and_determinism(gq):
         counts[b] = 1
         counts[0] = K - 1
         a = gq.grinqh_assign(_dev(x), counts)
-        y = gq.grinqh_vmm(_dev(x), w, a).cpu().numpy()
+        y = gq.grinqh_vmm(w, a).cpu().numpy()
         y_ref = oracle.dequant(planes, s, z, b)[k]
         assert np.allclose(y[0], y_ref, rtol=1e-6, atol=1e-9)
     x = synth.make_x(1, K, 32)
     counts = oracle.mix_to_counts(K, synth.MIXES["4"])
     xd = _dev(x)
     a = gq.grinqh_assign(xd, counts)
-    y1 = gq.grinqh_vmm(xd, w, a).cpu().numpy()
-    y2 = gq.grinqh_vmm(xd, w, a).cpu().numpy()
+    y1 = gq.grinqh_vmm(w, a).cpu().numpy()
+    y2 = gq.grinqh_vmm(w, a).cpu().numpy()
     assert np.array_equal(y1, y2)                   # deterministic split-K
 
 
@@ -195,10 +196,10 @@ def test_full_size_layer_sampled_columns(gq):
     xd = _dev(x)
     w = gq.grinqh_pack(Wd)
     a = gq.grinqh_assign(xd, counts)
-    y = gq.grinqh_vmm(xd, w, a)
+    y = gq.grinqh_vmm(w, a)
     torch.cuda.synchronize()
     ref_a = oracle.assign(x, counts)
-    _check_assign(ref_a, a)
+    _check_assign(ref_a, a, x)
     cols = np.unique(np.concatenate([np.arange(0, 64), np.arange(N - 64, N),
                                      np.random.default_rng(0).integers(0, N, 160)])).astype(np.int32)
     blocks = np.unique(cols // 32)

@@ -62,16 +62,16 @@ def test_argument_validation_without_gpu(lib):
     assert lib.grinqh_pack(16, 128, 40, 128, 16, 16, 16, None) == -2                  # N % 32
     assert lib.grinqh_pack(16, 128, 32, 64, 16, 16, 16, None) == -2                   # group
     assert lib.grinqh_pack(8, 128, 32, 128, 16, 16, 16, None) == -3                   # alignment
-    lib.grinqh_assign.argtypes = [vp, C.c_int, C.c_int, vp] + [vp] * 6 + [vp, C.c_size_t, vp]
+    lib.grinqh_assign.argtypes = [vp, C.c_int, C.c_int, vp] + [vp] * 7 + [vp, C.c_size_t, vp]
     counts = (C.c_uint32 * 9)(1, 0, 0, 0, 0, 0, 0, 0, 100)
-    assert lib.grinqh_assign(16, 1, 128, counts, 16, 16, 16, 16, 16, 16, None, 0, None) == -4   # sum != K
-    assert lib.grinqh_assign(16, 5, 128, counts, 16, 16, 16, 16, 16, 16, None, 0, None) == -2   # T
+    assert lib.grinqh_assign(16, 1, 128, counts, 16, 16, 16, 16, 16, 16, 16, None, 0, None) == -4   # sum != K
+    assert lib.grinqh_assign(16, 5, 128, counts, 16, 16, 16, 16, 16, 16, 16, None, 0, None) == -2   # T
     lib.grinqh_vmm_workspace_bytes.restype = C.c_size_t
     lib.grinqh_vmm_workspace_bytes.argtypes = [C.c_int] * 3
     assert lib.grinqh_vmm_workspace_bytes(1, 4096, 4096) > 0
     assert lib.grinqh_vmm_workspace_bytes(1, 4000, 4096) == 0
-    lib.grinqh_vmm.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.c_int] + [vp] * 7 + [vp, vp, C.c_size_t, vp]
-    assert lib.grinqh_vmm(16, 1, 128, 32, 128, 16, 16, 16, 16, 16, 16, 16, 16, 16, 0, None) == -5  # workspace
+    lib.grinqh_vmm.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int] + [vp] * 5 + [vp, vp, C.c_size_t, vp]
+    assert lib.grinqh_vmm(1, 128, 32, 128, 16, 16, 16, 16, 16, 16, 16, 0, None) == -5  # workspace
 
 
 def test_gather_network_on_host(tmp_path):
