@@ -1,28 +1,40 @@
-// assign.cu — grinqh_assign: |x| ranking -> per-channel bit widths -> compacted row lists (v2).
+// assign.cu — grinqh_assign: |x| ranking -> per-channel bit widths -> compacted row lists (v3).
 // PAPER.md:61-65 (assignment), :271 (top-p partition of the live vector); readings #2-#4.
 //
-// One CTA of 1024 threads, no sort.  Per token a two-level radix select on the 15-bit fp16 magnitude:
-//   level 1  256-bin histogram of key >> 7 (8 sub-histograms against atomic contention); one warp scans it
-//            from the top and finds, for each of the (at most 8) cuts C_w, the bin that contains it;
-//   level 2  128-bin histograms of key & 127 restricted to those bins; warp w finds the exact cut key thr_w,
-//            how many of the keys equal to thr_w are still inside (take_w), and whether the cut splits a run
-//            of equal keys.
-// Widths are then b = #{w : key >= thr_w}.  Only if some cut splits a tie run (ties go to the lower index) an
-// ordered count of the equal keys (per 128-row group, then a scan over groups) decides them.
-// Lists: one warp per 128-row group partitions its rows by (width desc, index asc) with ballots -> grows,
-// gcnt_ge, gsched; a scan over the groups' per-width counts places every group's runs in the global `rows`.
+// One thread-block cluster of 8 CTAs x 512 threads (8 SMs: a single SM is compute-bound on this, ~400 lane-ops
+// per key), no sort and no shared-memory atomics (measured here: ~2.3 ns per key per pass, the LSU serialises
+// them per lane; ballot-matching inside a warp costs as much in issue slots).  Counting is THREAD-PRIVATE instead:
+// thread t owns byte column t of cnt[slot][digit][512], so a histogram update is a plain LDS/ADD/STS with no
+// conflicts; a row is summed afterwards with dp4a, the 8 CTAs' row sums are read through DSMEM and every CTA
+// takes the same decisions on its own copy (no central CTA, one cluster barrier per level).
+// Per token a radix select on the 15-bit fp16 magnitude, 3 + 4 + 4 + 4 bits from the top: every distinct cut
+// C_d keeps (prefix, rank still needed inside the prefix); cuts with the same prefix share a histogram slot.
+// After the last level thr_d is the exact cut key, take_d how many of the keys equal to thr_d are inside, and
+// the cut "splits" if take_d is smaller than their number (ties go to the lower index): only then an ordered
+// count of the equal keys (per 128-row group, then a scan over groups) decides them.  fp16 has few distinct
+// magnitudes, so splits are the common case, not the exception.
+// Widths: b = sum_d mult_d [key above cut d].  Lists: one warp per 128-row group partitions its rows by
+// (width desc, index asc) with ballots -> grows, gcnt_ge, gsched; a scan over the groups' per-width counts
+// places every group's runs in the global `rows`.
+#include <cooperative_groups.h>
+
 #include "common.cuh"
+
+namespace cg = cooperative_groups;
 
 namespace gq {
 
-constexpr int AT = 1024;  // threads
+constexpr int AT = 512;   // threads per CTA
 constexpr int AWARPS = AT / 32;
-constexpr int NSUB = 8;
-constexpr int MAXG = GQ_MAX_K / GQ_G;  // 256 groups
+constexpr int MAXG = GQ_MAX_K / GQ_G;     // 256 groups
+constexpr int CNT_BYTES = 8 * 16 * AT;    // cnt[8 slots][16 digits][1024 thread columns] u8
 
 struct AssignParams {
     int T, K;
-    int C[10];  // C[w] = rows with width >= w (C[0] = K, C[9] = 0)
+    int nd;       // distinct non-zero cuts
+    int Cd[8];    // their ranks: the Cd[d] largest keys are "above" cut d
+    int mult[8];  // how many widths w share the cut: b = sum_d mult[d] * [above cut d]
+    int C[10];    // C[w] = rows with width >= w (for cnt_ge bookkeeping only)
 };
 
 __device__ __forceinline__ int warp_incl_scan(int v, int lane) {
@@ -34,8 +46,8 @@ __device__ __forceinline__ int warp_incl_scan(int v, int lane) {
     return v;
 }
 
-// tab[g][col], g < groups: exclusive prefix over g, in place; returns the total to lane 31's caller via *tot.
-// One warp per column; lane l owns groups 8l..8l+7.
+// tab[g][col], g < groups: exclusive prefix over g, in place; *tot = total.  One warp per column;
+// lane l owns groups 8l..8l+7.
 __device__ __forceinline__ void scan_groups(uint16_t (*tab)[10], int col, int groups, int lane, int* tot) {
     int v[8], s = 0;
 #pragma unroll
@@ -55,204 +67,208 @@ __device__ __forceinline__ void scan_groups(uint16_t (*tab)[10], int col, int gr
     if (lane == 31) *tot = incl;
 }
 
-__global__ void __launch_bounds__(AT, 1)
+constexpr int NC = 8;             // CTAs in the cluster (portable maximum); CTA r owns a contiguous run of groups
+constexpr int MAXLG = MAXG / NC;  // groups per CTA
+
+__global__ void __cluster_dims__(NC, 1, 1) __launch_bounds__(AT, 1)
 assign_kernel(const uint16_t* __restrict__ x, AssignParams p, uint8_t* __restrict__ bits,
               uint8_t* __restrict__ bits_union, int32_t* __restrict__ rows, int32_t* __restrict__ cnt_ge,
               uint8_t* __restrict__ grows, uint8_t* __restrict__ gcnt_ge, uint32_t* __restrict__ gsched) {
-    extern __shared__ __align__(16) uint8_t smem[];
-    uint16_t* keys = reinterpret_cast<uint16_t*>(smem);  // K u16 (current token); later aliased by glist (K u8)
-    uint8_t* glist = smem;
-    uint8_t* ubits = smem + (size_t)p.K * 2;             // K u8, union of the token widths
-    __shared__ uint32_t hist1[NSUB][256];
-    __shared__ uint32_t hist2[8][128];
-    __shared__ uint16_t tab[MAXG][10];
-    __shared__ int s_B[9], s_above[9], s_thr[9], s_take[9], s_split[9], s_tot[10];
-    __shared__ int s_anysplit;
+    cg::cluster_group cluster = cg::this_cluster();
+    const int rank = (int)cluster.block_rank();
+    extern __shared__ __align__(16) uint8_t cnt[];                  // [8][16][AT] u8 thread-private counters
+    __shared__ __align__(16) uint16_t xs[MAXLG * GQ_G];             // raw fp16 patterns, local groups, current token
+    __shared__ __align__(16) uint8_t glist[MAXLG * GQ_G];
+    __shared__ __align__(16) uint8_t gcs[MAXLG][GQ_GCNT];
+    __shared__ uint16_t tab[MAXG][10];                              // replicated: every CTA holds all groups
+    __shared__ int s_rowL[4][8 * 16];                               // this CTA's row sums, one array per level
+    __shared__ int s_row[8 * 16];                                   // cluster-wide row sums of the current level
+    __shared__ int s_pre[8], s_need[8], s_h[8], s_tot[10];
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int K = p.K, groups = K / GQ_G;
+    const int K = p.K, groups = K / GQ_G, nd = p.nd;
+    const int gpc = (groups + NC - 1) / NC;
+    const int gl0 = rank * gpc;                                     // first local group
+    const int nloc = max(0, min(gpc, groups - gl0));
     const uint32_t lt_mask = (1u << lane) - 1u;
 
+    auto zero_cnt = [&]() {
+        uint4* z = reinterpret_cast<uint4*>(cnt);
+#pragma unroll
+        for (int i = 0; i < CNT_BYTES / 16 / AT; ++i) z[tid + i * AT] = make_uint4(0, 0, 0, 0);
+    };
+
     for (int t = 0; t < p.T; ++t) {
-        // ---- P0: clear, keys, level-1 histogram
-        for (int i = tid; i < NSUB * 256; i += AT) (&hist1[0][0])[i] = 0;
-        (&hist2[0][0])[tid] = 0;
-        if (tid < 9) {
-            s_B[tid] = -1;
-            s_above[tid] = 0;
-            s_thr[tid] = 0x8000;  // above every key: no channel reaches this width
-            s_take[tid] = 0;
-            s_split[tid] = 0;
-        }
-        if (tid == 0) s_anysplit = 0;
-        __syncthreads();
-        {
-            const uint32_t* x2 = reinterpret_cast<const uint32_t*>(x + (size_t)t * K);
-            uint32_t* h = hist1[warp & (NSUB - 1)];
-            for (int i = tid; i < K / 2; i += AT) {
-                const uint32_t v = x2[i] & 0x7FFF7FFFu;
-                reinterpret_cast<uint32_t*>(keys)[i] = v;
-                atomicAdd(&h[(v & 0xFFFFu) >> 7], 1u);
-                atomicAdd(&h[v >> 23], 1u);
-            }
+        // ---- load the token's local groups (raw patterns; the key is pattern & 0x7FFF)
+        for (int i = tid; i < nloc * (GQ_G / 4); i += AT)
+            reinterpret_cast<uint2*>(xs)[i] = reinterpret_cast<const uint2*>(x + (size_t)t * K + gl0 * GQ_G)[i];
+        zero_cnt();
+        if (tid < 8) {
+            s_pre[tid] = 0;
+            s_need[tid] = (tid < nd) ? p.Cd[tid] : 0;
+            s_h[tid] = 0;
         }
         __syncthreads();
-        // ---- P1: warp 0 scans the 256 bins from the top and locates the bin of every cut
-        if (warp == 0) {
-            int h[8], s = 0;
+
+        // ---- radix select, 3 + 4 + 4 + 4 bits
+#pragma unroll 1
+        for (int level = 0; level < 4; ++level) {
+            const int nb = level ? 4 : 3;
+            const int sh = 12 - 4 * level;
+            int pre[8], slot[8];
 #pragma unroll
-            for (int i = 0; i < 8; ++i) {
-                const int bin = 255 - 8 * lane - i;
-                int c = 0;
+            for (int d = 0; d < 8; ++d) pre[d] = (d < nd) ? s_pre[d] : -1 - d;
 #pragma unroll
-                for (int u = 0; u < NSUB; ++u) c += (int)hist1[u][bin];
-                h[i] = c;
-                s += c;
+            for (int d = 0; d < 8; ++d) {
+                slot[d] = d;
+#pragma unroll
+                for (int e = d - 1; e >= 0; --e)
+                    if (pre[e] == pre[d]) slot[d] = e;
             }
-            const int above = warp_incl_scan(s, lane) - s;
+            // pass: count the digit of every local key whose prefix is a live one, in this thread's own columns
+            for (int i = tid; i < nloc * GQ_G; i += AT) {
+                const uint32_t m = xs[i] & 0x7FFFu;
+                const int pe = (int)(m >> (sh + nb));
+                int s = -1;
 #pragma unroll
-            for (int w = 1; w <= 8; ++w) {
-                const int Cw = p.C[w];
-                if (Cw > 0 && above < Cw && Cw <= above + s) {
-                    int run = above;
-                    bool done = false;
-#pragma unroll
-                    for (int i = 0; i < 8; ++i) {
-                        if (!done && Cw <= run + h[i]) {
-                            s_B[w] = 255 - 8 * lane - i;
-                            s_above[w] = run;
-                            done = true;
-                        }
-                        run += h[i];
-                    }
+                for (int d = 7; d >= 0; --d)
+                    if (slot[d] == d && pe == pre[d]) s = d;
+                if (s >= 0) {
+                    uint8_t* c = cnt + ((s * 16 + (int)((m >> sh) & ((1u << nb) - 1u))) * AT + tid);
+                    *c = (uint8_t)(*c + 1);
                 }
             }
-        }
-        __syncthreads();
-        // ---- P2: level-2 histograms inside the cut bins (cuts that share a bin share histogram `slot`)
-        int B[9], slot[9];
+            __syncthreads();
+            // reduce: a warp sums one row (AT bytes) of the live slots
+            for (int r = warp; r < nd * 16; r += AWARPS) {
+                const uint4 a = reinterpret_cast<const uint4*>(cnt + r * AT)[lane];
+                uint32_t s = 0;
+                s = __dp4a(a.x, 0x01010101u, s); s = __dp4a(a.y, 0x01010101u, s);
+                s = __dp4a(a.z, 0x01010101u, s); s = __dp4a(a.w, 0x01010101u, s);
+                s = __reduce_add_sync(0xffffffffu, s);
+                if (lane == 0) s_rowL[level][r] = (int)s;
+            }
+            cluster.sync();
+            // gather the 8 CTAs' row sums (DSMEM), then every CTA takes the same decisions on its own copy
+            if (tid < nd * 16) {
+                int s = 0;
 #pragma unroll
-        for (int w = 1; w <= 8; ++w) B[w] = s_B[w];
+                for (int r = 0; r < NC; ++r) s += cluster.map_shared_rank(&s_rowL[0][0], r)[level * 128 + tid];
+                s_row[tid] = s;
+            }
+            if (level < 3) zero_cnt();
+            __syncthreads();
+            if (warp < nd) {
+                const int d = warp;
+                int sl = 0;
 #pragma unroll
-        for (int w = 1; w <= 8; ++w) {
-            slot[w] = w;
-#pragma unroll
-            for (int v = w - 1; v >= 1; --v)
-                if (B[v] == B[w]) slot[w] = v;
-        }
-        for (int i = tid; i < K; i += AT) {
-            const int m = keys[i];
-            const int top = m >> 7;
-#pragma unroll
-            for (int w = 1; w <= 8; ++w)
-                if (top == B[w] && slot[w] == w) atomicAdd(&hist2[w - 1][m & 127], 1u);
-        }
-        __syncthreads();
-        // ---- P3: warp w-1 finds the exact cut key of cut w
-        if (warp < 8) {
-            const int w = warp + 1;
-            int Bw = -1, sl = 1, ab = 0;
-#pragma unroll
-            for (int v = 1; v <= 8; ++v)
-                if (v == w) { Bw = B[v]; sl = slot[v]; }
-            ab = s_above[w];
-            if (Bw >= 0) {
-                const int need = p.C[w] - ab;  // 1 <= need <= keys in bin Bw
-                int h[4], s = 0;
-#pragma unroll
-                for (int i = 0; i < 4; ++i) {
-                    h[i] = (int)hist2[sl - 1][127 - 4 * lane - i];
-                    s += h[i];
-                }
-                const int above = warp_incl_scan(s, lane) - s;
-                if (above < need && need <= above + s) {
-                    int run = above;
-                    bool done = false;
-#pragma unroll
-                    for (int i = 0; i < 4; ++i) {
-                        if (!done && need <= run + h[i]) {
-                            s_thr[w] = (Bw << 7) | (127 - 4 * lane - i);
-                            s_take[w] = need - run;
-                            if (need - run < h[i]) {
-                                s_split[w] = 1;
-                                s_anysplit = 1;
-                            }
-                            done = true;
-                        }
-                        run += h[i];
-                    }
+                for (int e = 0; e < 8; ++e)
+                    if (e == d) sl = slot[e];
+                const int digit = (1 << nb) - 1 - lane;
+                const int h = (digit >= 0) ? s_row[sl * 16 + digit] : 0;
+                const int incl = warp_incl_scan(h, lane);
+                const int above = incl - h, need = s_need[d], pr = s_pre[d];
+                __syncwarp();
+                if (above < need && need <= above + h) {
+                    s_pre[d] = (pr << nb) | digit;
+                    s_need[d] = need - above;
+                    s_h[d] = h;
                 }
             }
+            __syncthreads();
         }
-        __syncthreads();
-        int thr[9], take[9], split[9];
+        int thr[8], take[8], mult[8];
+        bool split[8], anysplit = false;
 #pragma unroll
-        for (int w = 1; w <= 8; ++w) {
-            thr[w] = s_thr[w];
-            take[w] = s_take[w];
-            split[w] = s_split[w];
+        for (int d = 0; d < 8; ++d) {
+            thr[d] = (d < nd) ? s_pre[d] : 0x8000;
+            take[d] = (d < nd) ? s_need[d] : 0;
+            mult[d] = (d < nd) ? p.mult[d] : 0;
+            split[d] = (d < nd) && take[d] < s_h[d];
+            anysplit |= split[d];
         }
-        const bool anysplit = s_anysplit != 0;
-        if (anysplit) {
-            // ---- a cut splits a run of equal keys: ordered (index-ascending) count of the equal keys
-            for (int g = warp; g < groups; g += AWARPS) {
-                const uint2 kv = *reinterpret_cast<const uint2*>(keys + g * GQ_G + 4 * lane);
-                const int m[4] = {(int)(kv.x & 0xFFFF), (int)(kv.x >> 16), (int)(kv.y & 0xFFFF), (int)(kv.y >> 16)};
+        if (anysplit) {  // cluster-uniform
+            // ---- a cut splits a run of equal keys: ordered (index-ascending) count of the equal keys;
+            //      every CTA gets every group's count (remote stores), then scans its own copy
+            for (int lg = warp; lg < nloc; lg += AWARPS) {
+                const uint2 kv = *reinterpret_cast<const uint2*>(xs + lg * GQ_G + 4 * lane);
+                const int m[4] = {(int)(kv.x & 0x7FFF), (int)((kv.x >> 16) & 0x7FFF), (int)(kv.y & 0x7FFF),
+                                  (int)((kv.y >> 16) & 0x7FFF)};
+                int mine = 0;
 #pragma unroll
-                for (int w = 1; w <= 8; ++w)
-                    if (split[w]) {
+                for (int d = 0; d < 8; ++d)
+                    if (split[d]) {
                         int c = 0;
 #pragma unroll
-                        for (int i = 0; i < 4; ++i) c += (m[i] == thr[w]);
+                        for (int i = 0; i < 4; ++i) c += (m[i] == thr[d]);
                         c = __reduce_add_sync(0xffffffffu, c);
-                        if (lane == 0) tab[g][w] = (uint16_t)c;
+                        if ((lane & 7) == d) mine = c;
                     }
+                // lane = 8 * r' + d (r' < 4) stores column d to CTAs r' and r' + 4
+                if (split[lane & 7]) {
+                    cluster.map_shared_rank(&tab[0][0], lane >> 3)[(gl0 + lg) * 10 + (lane & 7)] = (uint16_t)mine;
+                    cluster.map_shared_rank(&tab[0][0], (lane >> 3) + 4)[(gl0 + lg) * 10 + (lane & 7)] = (uint16_t)mine;
+                }
             }
-            __syncthreads();
-            if (warp < 8 && split[warp + 1]) {
+            cluster.sync();
+            if (warp < 8 && split[warp]) {
                 int dummy;
-                scan_groups(tab, warp + 1, groups, lane, &dummy);
+                scan_groups(tab, warp, groups, lane, &dummy);
             }
             __syncthreads();
         }
-        // ---- P4: widths of this token
-        for (int g = warp; g < groups; g += AWARPS) {
-            const uint2 kv = *reinterpret_cast<const uint2*>(keys + g * GQ_G + 4 * lane);
-            const int m[4] = {(int)(kv.x & 0xFFFF), (int)(kv.x >> 16), (int)(kv.y & 0xFFFF), (int)(kv.y >> 16)};
+        // ---- widths of this token
+        for (int lg = warp; lg < nloc; lg += AWARPS) {
+            const int g = gl0 + lg;
+            const uint2 kv = *reinterpret_cast<const uint2*>(xs + lg * GQ_G + 4 * lane);
+            const int m[4] = {(int)(kv.x & 0x7FFF), (int)((kv.x >> 16) & 0x7FFF), (int)(kv.y & 0x7FFF),
+                              (int)((kv.y >> 16) & 0x7FFF)};
             int b[4] = {0, 0, 0, 0};
 #pragma unroll
-            for (int w = 1; w <= 8; ++w) {
-                if (!split[w]) {
+            for (int d = 0; d < 8; ++d) {
+                if (!split[d]) {
 #pragma unroll
-                    for (int i = 0; i < 4; ++i) b[i] += (m[i] >= thr[w]);
+                    for (int i = 0; i < 4; ++i) b[i] += (m[i] >= thr[d]) ? mult[d] : 0;
                 } else {
                     bool eq[4];
-                    int below = tab[g][w];  // equal keys in earlier groups
+                    int below = tab[g][d];  // equal keys in earlier groups
 #pragma unroll
                     for (int i = 0; i < 4; ++i) {
-                        eq[i] = (m[i] == thr[w]);
+                        eq[i] = (m[i] == thr[d]);
                         below += __popc(__ballot_sync(0xffffffffu, eq[i]) & lt_mask);
                     }
 #pragma unroll
                     for (int i = 0; i < 4; ++i) {
-                        b[i] += (m[i] > thr[w]) || (eq[i] && below < take[w]);
+                        b[i] += ((m[i] > thr[d]) || (eq[i] && below < take[d])) ? mult[d] : 0;
                         below += eq[i];
                     }
                 }
             }
             const uint32_t packed = (uint32_t)b[0] | ((uint32_t)b[1] << 8) | ((uint32_t)b[2] << 16) | ((uint32_t)b[3] << 24);
             *reinterpret_cast<uint32_t*>(bits + (size_t)t * K + g * GQ_G + 4 * lane) = packed;
-            uint32_t* u = reinterpret_cast<uint32_t*>(ubits + g * GQ_G + 4 * lane);
-            *u = (t == 0) ? packed : __vmaxu4(*u, packed);
+            uint32_t* u = reinterpret_cast<uint32_t*>(bits_union + g * GQ_G + 4 * lane);  // same thread every token
+            if (t == 0) *u = packed;
+            else *u = __vmaxu4(*u, packed);
         }
-        __syncthreads();
+        // tab is rewritten remotely by the next token / the width counts: everybody must be done reading it
+        if (anysplit) cluster.sync();
+        else __syncthreads();
     }
 
-    // ---- P5: per-group lists (keys are dead: glist aliases them)
-    __shared__ __align__(16) uint8_t gcs[MAXG][GQ_GCNT];
-    for (int g = warp; g < groups; g += AWARPS) {
-        const uint32_t bu4 = *reinterpret_cast<const uint32_t*>(ubits + g * GQ_G + 4 * lane);
-        *reinterpret_cast<uint32_t*>(bits_union + g * GQ_G + 4 * lane) = bu4;
+    // ---- per-group lists of the local groups
+    for (int lg = warp; lg < nloc; lg += AWARPS) {
+        const int g = gl0 + lg;
+        const int go = g * GQ_G + 4 * lane, lo = lg * GQ_G + 4 * lane;
+        const uint32_t bu4 = *reinterpret_cast<const uint32_t*>(bits_union + go);
+        uint32_t bt4[GRINQH_MAX_T];
+        uint2 xv[GRINQH_MAX_T];
+#pragma unroll
+        for (int t = 0; t < GRINQH_MAX_T; ++t)
+            if (t < p.T) {
+                bt4[t] = (p.T == 1) ? bu4 : *reinterpret_cast<const uint32_t*>(bits + (size_t)t * K + go);
+                xv[t] = (p.T == 1) ? *reinterpret_cast<const uint2*>(xs + lo)
+                                   : *reinterpret_cast<const uint2*>(x + (size_t)t * K + go);
+            }
         int bu[4], pos[4];
 #pragma unroll
         for (int i = 0; i < 4; ++i) bu[i] = (bu4 >> (8 * i)) & 0xFF;
@@ -278,29 +294,34 @@ assign_kernel(const uint16_t* __restrict__ x, AssignParams p, uint8_t* __restric
         if (lane < GQ_GCNT) {
             const uint8_t v = (uint8_t)(lane <= 8 ? myge : 0);
             gcnt_ge[g * GQ_GCNT + lane] = v;
-            gcs[g][lane] = v;
+            gcs[lg][lane] = v;
         }
-        if (lane < 9) tab[g][lane] = (uint16_t)myn;
-#pragma unroll
-        for (int i = 0; i < 4; ++i) glist[g * GQ_G + pos[i]] = (uint8_t)(4 * lane + i);
-        for (int t = 0; t < p.T; ++t) {
-            const uint32_t bt4 = *reinterpret_cast<const uint32_t*>(bits + (size_t)t * K + g * GQ_G + 4 * lane);
-            const uint2 xv = *reinterpret_cast<const uint2*>(x + (size_t)t * K + g * GQ_G + 4 * lane);
-            const uint32_t xs[4] = {xv.x & 0xFFFFu, xv.x >> 16, xv.y & 0xFFFFu, xv.y >> 16};
-#pragma unroll
-            for (int i = 0; i < 4; ++i)
-                gsched[(size_t)t * K + g * GQ_G + pos[i]] = (uint32_t)(4 * lane + i) | (((bt4 >> (8 * i)) & 0xFFu) << 8) |
-                                                            ((uint32_t)bu[i] << 12) | (xs[i] << 16);
+        {   // every CTA gets the group's 9 per-width counts: lane = 9 * r' + c stores column c to CTA r' (and r' + 3, r' + 6)
+            const int c = lane % 9, r0 = lane / 9;
+            const int n = __shfl_sync(0xffffffffu, myn, c);
+            if (lane < 27)
+                for (int r = r0; r < NC; r += 3) cluster.map_shared_rank(&tab[0][0], r)[g * 10 + c] = (uint16_t)n;
         }
+#pragma unroll
+        for (int i = 0; i < 4; ++i) glist[lg * GQ_G + pos[i]] = (uint8_t)(4 * lane + i);
+#pragma unroll
+        for (int t = 0; t < GRINQH_MAX_T; ++t)
+            if (t < p.T) {
+                const uint32_t xq[4] = {xv[t].x & 0xFFFFu, xv[t].x >> 16, xv[t].y & 0xFFFFu, xv[t].y >> 16};
+#pragma unroll
+                for (int i = 0; i < 4; ++i)
+                    gsched[(size_t)t * K + g * GQ_G + pos[i]] = (uint32_t)(4 * lane + i) |
+                                                                (((bt4[t] >> (8 * i)) & 0xFFu) << 8) |
+                                                                ((uint32_t)bu[i] << 12) | (xq[i] << 16);
+            }
         __syncwarp();
-        *reinterpret_cast<uint32_t*>(grows + g * GQ_G + 4 * lane) =
-            *reinterpret_cast<const uint32_t*>(glist + g * GQ_G + 4 * lane);
+        *reinterpret_cast<uint32_t*>(grows + go) = *reinterpret_cast<const uint32_t*>(glist + lo);
     }
-    __syncthreads();
-    // ---- P6: where each group's run of every width starts in the global list
+    cluster.sync();  // the last remote access of the kernel is before this barrier
+    // ---- where each group's run of every width starts in the global list (every CTA scans its own copy)
     if (warp < 9) scan_groups(tab, warp, groups, lane, &s_tot[warp]);
     __syncthreads();
-    // ---- P7: global list (width desc, index asc) and cnt_ge
+    // ---- global list (width desc, index asc) and cnt_ge
     int cbase[9];
     {
         int acc = 0;
@@ -310,13 +331,14 @@ assign_kernel(const uint16_t* __restrict__ x, AssignParams p, uint8_t* __restric
             acc += s_tot[c];
         }
     }
-    if (tid < 10) cnt_ge[tid] = (tid == 9) ? 0 : cbase[tid] + s_tot[tid];
-    for (int g = warp; g < groups; g += AWARPS) {
-        const uint4 cv = *reinterpret_cast<const uint4*>(gcs[g]);
+    if (rank == 0 && tid < 10) cnt_ge[tid] = (tid == 9) ? 0 : cbase[tid] + s_tot[tid];
+    for (int lg = warp; lg < nloc; lg += AWARPS) {
+        const int g = gl0 + lg;
+        const uint4 cv = *reinterpret_cast<const uint4*>(gcs[lg]);
         const int cge[10] = {(int)(cv.x & 0xFF), (int)((cv.x >> 8) & 0xFF), (int)((cv.x >> 16) & 0xFF), (int)(cv.x >> 24),
                              (int)(cv.y & 0xFF), (int)((cv.y >> 8) & 0xFF), (int)((cv.y >> 16) & 0xFF), (int)(cv.y >> 24),
                              (int)(cv.z & 0xFF), 0};
-        const uint32_t l4 = *reinterpret_cast<const uint32_t*>(glist + g * GQ_G + 4 * lane);
+        const uint32_t l4 = *reinterpret_cast<const uint32_t*>(glist + lg * GQ_G + 4 * lane);
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
             const int pp = 4 * lane + i;
@@ -351,20 +373,30 @@ extern "C" int grinqh_assign(const void* x_f16, int T, int K, const uint32_t cou
     unsigned long long total = 0;
     for (int w = 0; w < 9; ++w) total += counts[w];
     if (total != (unsigned long long)K) return GRINQH_ERR_MIX;
-    gq::AssignParams p;
+    gq::AssignParams p{};
     p.T = T;
     p.K = K;
     p.C[9] = 0;
     for (int w = 8; w >= 0; --w) p.C[w] = p.C[w + 1] + (int)counts[w];
-    const size_t smem = (size_t)K * 3;
+    for (int w = 1; w <= 8; ++w) {  // distinct non-zero cuts
+        if (p.C[w] == 0) continue;
+        int d = 0;
+        while (d < p.nd && p.Cd[d] != p.C[w]) ++d;
+        if (d == p.nd) {
+            p.Cd[p.nd] = p.C[w];
+            p.mult[p.nd++] = 0;
+        }
+        p.mult[d]++;
+    }
+    const size_t smem = (size_t)gq::CNT_BYTES;
     static bool configured = false;
     if (!configured) {
-        if (cudaFuncSetAttribute(gq::assign_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, GQ_MAX_K * 3) !=
-            cudaSuccess)
+        if (cudaFuncSetAttribute(gq::assign_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 gq::CNT_BYTES) != cudaSuccess)
             return GRINQH_ERR_CUDA;
         configured = true;
     }
-    gq::assign_kernel<<<1, gq::AT, smem, (cudaStream_t)stream>>>((const uint16_t*)x_f16, p, bits, bits_union, rows,
+    gq::assign_kernel<<<gq::NC, gq::AT, smem, (cudaStream_t)stream>>>((const uint16_t*)x_f16, p, bits, bits_union, rows,
                                                                 cnt_ge, grows, gcnt_ge, gsched);
     return cudaGetLastError() == cudaSuccess ? GRINQH_OK : GRINQH_ERR_CUDA;
 }
