@@ -3,8 +3,9 @@
 
 Workload (N = 1): BASELINE.json configs[1] — one Llama-3-8B-shaped layer, batch 1, avg 4 bits:
 7 projections (q,k,v,o,gate,up,down), 4 distinct input vectors (q/k/v and gate/up share one).
-A "step" = one pass of the per-step hot path over one layer: 4 x grinqh_assign + 7 x grinqh_vmm
-(main + reduce).  grinqh_pack is offline (once per weight) and reported separately under "pack".
+A "step" = one pass of the per-step hot path over one layer: 4 x grinqh_assign + 4 x grinqh_vmm (q|k|v and
+gate|up concatenated along N; the deterministic split-K second pass runs inside the VMM launch).  The same step
+with one launch per projection (7 VMMs) is reported under "per_projection".  grinqh_pack is offline (once per weight) and reported separately under "pack".
 The timed loop rotates over LAYERS distinct packed layers (> L2) so every step streams from HBM.
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--mix 4] [--layers 4]
@@ -23,7 +24,7 @@ import time
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
-METRIC = "us per decode step of one Llama-3-8B-shaped layer (4 assigns + 7 bit-planar VMMs), batch 1"
+METRIC = "us per decode step of one Llama-3-8B-shaped layer (4 assigns + the 7 projections as bit-planar VMMs), batch 1"
 UNIT = "us"
 
 
@@ -37,6 +38,7 @@ def _args():
     ap.add_argument("--layers", type=int, default=4, help="distinct packed layers the timed loop rotates over")
     ap.add_argument("--seed", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-split", action="store_true", help="skip the one-launch-per-projection variant")
     return ap.parse_args()
 
 
@@ -192,18 +194,21 @@ def run_native(args):
     avg_bits = synth.mix_avg_bits(frac)
     L = args.layers
     T = 1
-    layer = synth.LLAMA3_8B_LAYER
+    fused = synth.LLAMA3_8B_LAYER_FUSED          # (name, K, N, input): the launches of the timed step
+    split = [(n, K, N, synth.LLAMA3_8B_INPUTS[n]) for n, K, N in synth.LLAMA3_8B_LAYER]
     in_dims = synth.LLAMA3_8B_INPUT_DIMS
     counts = {K: gq.grinqh_mix_to_counts(K, frac) for K in set(in_dims.values())}
 
     # ---- offline: generate + pack L distinct layers (grinqh_pack timed on its own)
     gen = torch.Generator(device=dev)
     gen.manual_seed(args.seed + 1000 * rank)
-    packed, pack_ms, pack_bytes = [], 0.0, 0
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    for l in range(L):
+    pack_ms, pack_bytes = 0.0, 0
+
+    def make_packed(shapes, timed):
+        nonlocal pack_ms, pack_bytes
         d = {}
-        for name, K, N in layer:
+        for name, K, N, _ in shapes:
             W = (torch.randn((K, N), generator=gen, device=dev, dtype=torch.float32) * 0.02).to(torch.float16)
             out = gq.Packed(K, N, dev)
             torch.cuda.synchronize()
@@ -211,48 +216,57 @@ def run_native(args):
             gq.grinqh_pack(W, out)
             e1.record()
             torch.cuda.synchronize()
-            pack_ms += e0.elapsed_time(e1)
-            pack_bytes += K * N * 3 + (K // 128) * N * 4
+            if timed:
+                pack_ms += e0.elapsed_time(e1)
+                pack_bytes += K * N * 3 + (K // 128) * N * 4
             d[name] = out
             del W
-        packed.append(d)
+        return d
+
+    packed = [make_packed(fused, True) for _ in range(L)]
+    packed_split = [make_packed(split, False) for _ in range(L)] if not args.no_split else None
 
     # ---- per-step inputs: fresh activations per layer copy (N(0,1), 1% channels x20)
     x_host = [{n: torch.from_numpy(synth.make_x(T, K, args.seed + 10 * l + i + 1000 * rank, "normal")).pin_memory()
                for i, (n, K) in enumerate(in_dims.items())} for l in range(L)]
     x_dev = [{n: v.to(dev) for n, v in xl.items()} for xl in x_host]
     assigns = [{n: gq.Assignment(T, K, dev) for n, K in in_dims.items()} for _ in range(L)]
-    y_dev = [{name: torch.empty((T, N), dtype=torch.float32, device=dev) for name, K, N in layer} for _ in range(L)]
-    y_host = [{name: torch.empty((T, N), dtype=torch.float32).pin_memory() for name, K, N in layer} for _ in range(L)]
-    ws_bytes = max(gq.grinqh_vmm_workspace_bytes(T, K, N) for _, K, N in layer)
-    ws = torch.empty((ws_bytes,), dtype=torch.uint8, device=dev)
+    all_shapes = list(fused) + split
+    y_dev = [{name: torch.empty((T, N), dtype=torch.float32, device=dev) for name, K, N, _ in all_shapes} for _ in range(L)]
+    y_host = [{name: torch.empty((T, N), dtype=torch.float32).pin_memory() for name, K, N, _ in fused} for _ in range(L)]
+    _, Kw, Nw, _ = max(all_shapes, key=lambda s: gq.grinqh_vmm_workspace_bytes(T, s[1], s[2]))
+    ws = gq.grinqh_vmm_workspace(T, Kw, Nw, dev)
     x_stage = {n: torch.empty((T, K), dtype=torch.float16, device=dev) for n, K in in_dims.items()}
 
-    def step_device(l):
-        for n, K in in_dims.items():
-            gq.grinqh_assign(x_dev[l][n], counts[K], assigns[l][n])
-        for name, K, N in layer:
-            n = synth.LLAMA3_8B_INPUTS[name]
-            gq.grinqh_vmm(packed[l][name], assigns[l][n], y_dev[l][name], ws)
+    def step_device(l):          # the timed step: 4 assigns + 4 VMM launches (qkv and gate/up concatenated)
+        for name, K, N, inp in fused:
+            gq.grinqh_assign(x_dev[l][inp], counts[K], assigns[l][inp])
+            gq.grinqh_vmm(packed[l][name], assigns[l][inp], y_dev[l][name], ws)
 
-    def step_main_only(l):
-        for name, K, N in layer:
-            n = synth.LLAMA3_8B_INPUTS[name]
-            gq.grinqh_vmm_main(packed[l][name], assigns[l][n], ws)
+    def step_split(l):           # the same step with one launch per projection: 4 assigns + 7 VMMs
+        seen = set()
+        for name, K, N, inp in split:
+            if inp not in seen:
+                gq.grinqh_assign(x_dev[l][inp], counts[K], assigns[l][inp])
+                seen.add(inp)
+            gq.grinqh_vmm(packed_split[l][name], assigns[l][inp], y_dev[l][name], ws)
+
+    def step_main_only(l):       # the dominant kernel alone: the 4 VMM launches (assignments already on the device)
+        for name, K, N, inp in fused:
+            gq.grinqh_vmm(packed[l][name], assigns[l][inp], y_dev[l][name], ws)
 
     def step_host(l):
-        seen = set()
-        for name, K, N in layer:
-            n = synth.LLAMA3_8B_INPUTS[name]
-            gq.grinqh_decode_host(x_host[l][n], counts[K], packed[l][name], assigns[l][n], x_stage[n],
-                                  y_dev[l][name], ws, y_host[l][name], reuse_assignment=(n in seen))
-            seen.add(n)
+        for name, K, N, inp in fused:
+            gq.grinqh_decode_host(x_host[l][inp], counts[K], packed[l][name], assigns[l][inp], x_stage[inp],
+                                  y_dev[l][name], ws, y_host[l][name], reuse_assignment=False)
 
     stream = torch.cuda.Stream(device=dev)
     with torch.cuda.stream(stream):
         for l in range(L):          # eager warm-up (also configures kernel attributes before capture)
             step_device(l)
             step_host(l)
+            if packed_split:
+                step_split(l)
         stream.synchronize()
 
         def capture(fn):
@@ -267,6 +281,7 @@ def run_native(args):
         g_dev = capture(step_device)
         g_main = capture(step_main_only)
         g_host = capture(step_host)
+        g_split = capture(step_split) if packed_split else None
 
         def barrier():
             if world > 1:
@@ -298,52 +313,62 @@ def run_native(args):
         for i in range(3):
             g_host[i % L].replay()
         ms_host = timed(g_host, args.steps, sync_each=True)
+        ms_split = None
+        if g_split:
+            for i in range(3):
+                g_split[i % L].replay()
+            ms_split = timed(g_split, args.steps)
 
     if world > 1:
         import torch.distributed as dist
-        t = torch.tensor([ms_total, ms_main, ms_host], device=dev, dtype=torch.float64)
+        t = torch.tensor([ms_total, ms_main, ms_host, ms_split or 0.0], device=dev, dtype=torch.float64)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total, ms_main, ms_host = [float(v) for v in t.tolist()]
+        ms_total, ms_main, ms_host, ms_split = [float(v) for v in t.tolist()]
 
-    # ---- algorithmic bytes of the 7 main-kernel launches of one step (measured widths)
+    # ---- algorithmic bytes of the VMM launches of one step (measured widths; SURVEY.md 8d / DESIGN.md)
     step_bytes, plane_bytes = 0, 0
     per_vmm = []
-    for name, K, N in layer:
-        n = synth.LLAMA3_8B_INPUTS[name]
-        sb = int(assigns[0][n].bits_union.sum().item())
+    for name, K, N, inp in fused:
+        sb = int(assigns[0][inp].bits_union.sum().item())
         b = alg_bytes(K, N, T, sb)
         step_bytes += b
         plane_bytes += (N // 8) * sb
-        per_vmm.append({"proj": name, "K": K, "N": N, "alg_bytes": b})
+        per_vmm.append({"launch": name, "K": K, "N": N, "alg_bytes": b})
     peak, peak_src = _peaks()
     us_step = ms_total * 1e3 / args.steps
     us_main = ms_main * 1e3 / args.steps
     us_host = ms_host * 1e3 / args.steps
-    achieved = step_bytes / (us_main * 1e-6) / 1e9  # GB/s over the 7 vmm_main launches of a step
+    achieved = step_bytes / (us_main * 1e-6) / 1e9  # GB/s over the VMM launches of a step
 
     h2d = sum(T * K * 2 for K in in_dims.values())
-    d2h = sum(T * N * 4 for _, _, N in layer)
+    d2h = sum(T * N * 4 for _, _, N, _ in fused)
+    weights = sum(K * N for _, K, N, _ in fused)
     line = {
         "metric": METRIC, "value": us_step / world, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": us_step / 1e3, "higher_is_better": False, "scaling": "weak",
         "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": "llama3-8b-layer (BASELINE.json configs[1]): 4096->4096 x2 (q,o), 4096->1024 x2 (k,v), "
                                "4096->14336 x2 (gate,up), 14336->4096 (down); batch 1; per-step rank assignment",
+                   "launches": "4 x grinqh_assign + 4 x grinqh_vmm per step: q|k|v and gate|up are concatenated along N "
+                               "(same input vector, per-column quantiser), the split-K second pass runs inside the VMM launch",
                    "avg_bits": avg_bits, "mix": args.mix, "group": 128, "tokens": T,
                    "l2": f"timed loop rotates over {L} distinct packed layers "
-                         f"({L * sum(K * N for _, K, N in layer) / 1e6:.0f} MB of planes > 126 MB L2); CUDA graph per layer",
+                         f"({L * weights / 1e6:.0f} MB of planes > 126 MB L2); one CUDA graph per layer",
                    "replicas": "replicas only (no data-path collective)" if world > 1 else "single GPU"},
         "clocks": clocks,
         "e2e": {"value": us_host / world, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                "how": "grinqh_decode_host per projection (pinned host x in, pinned host y out), stream sync per step"},
-        "gpu_launches": args.steps * (len(in_dims) + 2 * len(layer)),
+                "how": "grinqh_decode_host per launch (pinned host x in, pinned host y out), stream sync per step"},
+        "gpu_launches": args.steps * 2 * len(fused),
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": None, "kernel": "vmm_main_kernel<1> (7 launches per step)",
+                     "traffic": None, "kernel": f"vmm_main_kernel<1,1,1> ({len(fused)} launches per step)",
                      "alg_bytes_per_step": step_bytes, "plane_bytes_per_step": plane_bytes,
                      "us_per_step_main_only": us_main, "peak_source": peak_src},
         "pack": {"GBps": pack_bytes / (pack_ms * 1e-3) / 1e9, "ms_per_layer": pack_ms / L},
         "per_vmm": per_vmm,
     }
+    if ms_split:
+        line["per_projection"] = {"value": ms_split * 1e3 / args.steps, "unit": UNIT,
+                                  "what": "same step with one VMM launch per projection (4 assigns + 7 VMMs)"}
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         sample = OracleLayerSample(args.mix, args.seed, 1024)
         t = min(sample.run() for _ in range(3))

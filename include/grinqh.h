@@ -120,17 +120,22 @@ int grinqh_assign(const void* x_f16, int T, int K, const uint32_t counts[9],
 
 /*
  * grinqh_vmm — per projection (PAPER.md:85 reconstruction, :51 selective fetch).
- * Split-K main kernel (warps walk the per-group schedule and fetch only planes j < bits_union[k] of row k)
- * followed by a deterministic fixed-order second-pass reduce of the split-K partials.  fp32 accumulation.
+ * ONE launch: split-K main kernel (warps walk the per-group schedule and fetch only planes j < bits_union[k] of
+ * row k) whose last-finishing CTA per column tile runs the deterministic second pass: it sums the tile's split-K
+ * partials in the fixed order s = 0..S-1 (the result does not depend on which CTA is last).  fp32 accumulation.
  * For T > 1 each token is truncated to its own bits[t][k]; y[t] equals the T = 1 result of token t alone.
  * The activations enter through gsched (x values, widths and row order of the assignment).
  *   gsched, gcnt_ge   dev   as written by grinqh_assign for this [T, K] input
  *   y          dev  [T, N] fp32, written
- *   workspace  dev  >= grinqh_vmm_workspace_bytes(T, K, N) bytes, 16-byte aligned
- * grinqh_vmm_main / grinqh_vmm_reduce are the two halves (main writes the split-K partials into
- * workspace, reduce sums them into y); grinqh_vmm enqueues both.
+ *   workspace  dev  >= grinqh_vmm_workspace_bytes(T, K, N) bytes, 16-byte aligned.  Its first 16 KB hold the
+ *                   per-tile tickets: call grinqh_vmm_workspace_init ONCE after allocating it (and again only
+ *                   after an aborted launch); every launch leaves them zero.  One workspace may serve calls of
+ *                   different shapes as long as they are ordered on one stream (size it for the largest).
+ * grinqh_vmm_main / grinqh_vmm_reduce are the same computation as two launches (main writes the split-K partials
+ * into workspace, reduce sums them into y in the same fixed order); they do not use the tickets.
  */
 size_t grinqh_vmm_workspace_bytes(int T, int K, int N);
+int grinqh_vmm_workspace_init(void* workspace, size_t workspace_bytes, void* stream);
 int grinqh_vmm(int T, int K, int N, int group,
                const uint32_t* planes, const void* scales_f16, const void* zeros_f16,
                const uint32_t* gsched, const uint8_t* gcnt_ge,

@@ -39,6 +39,8 @@ _lib.grinqh_assign.restype = _i
 _lib.grinqh_assign.argtypes = [_vp, _i, _i, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _sz, _vp]
 _lib.grinqh_vmm_workspace_bytes.restype = _sz
 _lib.grinqh_vmm_workspace_bytes.argtypes = [_i, _i, _i]
+_lib.grinqh_vmm_workspace_init.restype = _i
+_lib.grinqh_vmm_workspace_init.argtypes = [_vp, _sz, _vp]
 _VMM_COMMON = [_i, _i, _i, _i, _vp, _vp, _vp, _vp, _vp]
 _lib.grinqh_vmm.restype = _i
 _lib.grinqh_vmm.argtypes = _VMM_COMMON + [_vp, _vp, _sz, _vp]
@@ -51,7 +53,8 @@ _lib.grinqh_decode_host.argtypes = [_vp, _i, _i, _i, _i, _vp, _vp, _vp, _vp, _vp
                                     _vp, _vp, _sz, _vp, _vp, _sz, _vp, _i, _vp]
 
 EXPORTS = ("grinqh_status_string", "grinqh_version", "grinqh_mix_to_counts", "grinqh_pack",
-           "grinqh_assign_workspace_bytes", "grinqh_assign", "grinqh_vmm_workspace_bytes", "grinqh_vmm",
+           "grinqh_assign_workspace_bytes", "grinqh_assign", "grinqh_vmm_workspace_bytes",
+           "grinqh_vmm_workspace_init", "grinqh_vmm",
            "grinqh_vmm_main", "grinqh_vmm_reduce", "grinqh_decode_host")
 
 
@@ -149,10 +152,16 @@ def _vmm_common(w: Packed, a: Assignment):
             a.gsched.data_ptr(), a.gcnt_ge.data_ptr()]
 
 
+def grinqh_vmm_workspace(T: int, K: int, N: int, device="cuda", stream=None) -> torch.Tensor:
+    """A workspace for shapes up to (T, K, N), tickets cleared (grinqh_vmm_workspace_init)."""
+    ws = torch.empty((grinqh_vmm_workspace_bytes(T, K, N),), dtype=torch.uint8, device=device)
+    _check(_lib.grinqh_vmm_workspace_init(ws.data_ptr(), ws.numel(), _stream(stream)), "grinqh_vmm_workspace_init")
+    return ws
+
+
 def _ws(T, K, N, workspace, device):
-    need = grinqh_vmm_workspace_bytes(T, K, N)
     if workspace is None:
-        workspace = torch.empty((max(need, 16),), dtype=torch.uint8, device=device)
+        workspace = grinqh_vmm_workspace(T, K, N, device)
     return workspace, workspace.numel() * workspace.element_size()
 
 

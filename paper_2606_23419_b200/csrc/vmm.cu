@@ -31,7 +31,7 @@ constexpr int TILE_COLS = 1024;
 constexpr int SLOT_BYTES = 1024;   // 8 planes x 128 B
 constexpr int YSLOT = 32 * 33;     // one warp's 1024 sums, padded: column 32*l + c lives at c*33 + l
 constexpr int NUM_SMS = 148;
-constexpr int CTAS_PER_SM = 2;
+constexpr int ctas_per_sm(int T) { return T <= 2 ? 2 : 1; }  // register / shared-memory budget
 
 template <int T>
 struct Cfg {
@@ -59,7 +59,7 @@ static inline VmmPlan vmm_plan(int T, int K, int N) {
     VmmPlan best{};
     const int CT = (N + TILE_COLS - 1) / TILE_COLS;
     const int groups = K / GQ_G;
-    const int resident = NUM_SMS * ((T <= 2) ? CTAS_PER_SM : 1);
+    const int resident = NUM_SMS * ctas_per_sm(T);
     const int sx_max = resident / CT > 0 ? resident / CT : 1;
     double best_cost = 1e30;
     for (int Q = 1; Q <= 8; ++Q) {
@@ -68,7 +68,7 @@ static inline VmmPlan vmm_plan(int T, int K, int N) {
         if (Sx > sx_max) Sx = sx_max;
         const int ipw = (I + VW * Sx - 1) / (VW * Sx);
         Sx = (I + VW * ipw - 1) / (VW * ipw);
-        const double cost = ipw * (112.0 / Q + 3.0);
+        const double cost = ipw * (112.0 / Q + 6.0);
         if (cost < best_cost - 1e-9) {
             best_cost = cost;
             best = VmmPlan{CT, Q, Sx, ipw};
@@ -109,12 +109,15 @@ __device__ __forceinline__ void accumulate_row(const uint32_t (&V)[8], uint16_t 
 //
 // gsched[t][g*128 + p] (written by grinqh_assign) is position p of group g's list for token t:
 //   bits 0..7 local row r | 8..11 b_t (token's width) | 12..15 b (union width = planes fetched) | 16..31 x_t[r] fp16
-template <int T, bool A16>
-__global__ void __launch_bounds__(VTHREADS, (T <= 2) ? CTAS_PER_SM : 1)
-vmm_main_kernel(int K, int N, int Q, int ipw, const uint32_t* __restrict__ planes,
+//
+// FUSED: the last CTA of a column tile to finish (ticket counter in the workspace, reset to 0 by that CTA) sums the
+// tile's Sx partials in the fixed order s = 0..Sx-1 and writes y: still deterministic, one launch instead of two.
+template <int T, bool A16, bool FUSED>
+__global__ void __launch_bounds__(VTHREADS, ctas_per_sm(T))
+vmm_main_kernel(int K, int N, int Q, uint32_t rq, int ipw, int Sx, const uint32_t* __restrict__ planes,
                 const __half* __restrict__ scales, const __half* __restrict__ zeros,
                 const uint32_t* __restrict__ gsched, const uint8_t* __restrict__ gcnt_ge,
-                float* __restrict__ part) {
+                float* __restrict__ part, int* __restrict__ tickets, float* __restrict__ y) {
     using C = Cfg<T>;
     constexpr int RING = C::RING;
     constexpr uint32_t RING_MASK = RING * SLOT_BYTES - 1;
@@ -150,12 +153,12 @@ vmm_main_kernel(int K, int N, int Q, int ipw, const uint32_t* __restrict__ plane
     bool first = true;
 
     for (int it = it0; it < it1; ++it) {
-        const int g = it / Q, q = it - g * Q;
+        const int g = (int)(((uint32_t)it * rq) >> 16), q = it - g * Q;  // it / Q (rq = ceil(65536 / Q), it < 8192)
         __syncwarp();
         // ---- item prologue: lane l stages item rows l, l+32, ... and the warp reduces X, Phi
         const uint4 cv = *reinterpret_cast<const uint4*>(gcnt_ge + g * GQ_GCNT);
         auto rows_ge = [&](uint32_t c) -> int {  // rows of this item among the first c list positions
-            return ((int)c > q) ? ((int)c - q + Q - 1) / Q : 0;
+            return ((int)c > q) ? (int)(((c - q + Q - 1) * rq) >> 16) : 0;
         };
         const int n_rows = rows_ge((cv.x >> 8) & 0xFF);
         float X[T], Phi[T];
@@ -330,7 +333,8 @@ vmm_main_kernel(int K, int N, int Q, int ipw, const uint32_t* __restrict__ plane
     }
     __syncthreads();
 
-    // ---- CTA epilogue: fixed-order sum over the 8 warps -> one split-K partial
+    // ---- CTA epilogue: fixed-order sum over the 8 warps -> one split-K partial (or y itself when Sx == 1)
+    float* out = (FUSED && Sx == 1) ? y : part + (size_t)sx * T * N;
 #pragma unroll
     for (int t = 0; t < T; ++t)
 #pragma unroll
@@ -343,67 +347,103 @@ vmm_main_kernel(int K, int N, int Q, int ipw, const uint32_t* __restrict__ plane
 #pragma unroll
                 for (int w = 0; w < VW; ++w)
                     A += *reinterpret_cast<const float*>(smem + w * C::WARP_BYTES + C::YACC_OFF + (t * YSLOT + idx) * 4);
-                part[((size_t)sx * T + t) * N + n] = A;
+                out[(size_t)t * N + n] = A;
             }
         }
+    if (FUSED && Sx > 1) {
+        __shared__ int s_last;
+        __threadfence();  // this CTA's partial is visible device-wide before its ticket
+        __syncthreads();
+        if (tid == 0) s_last = (atomicAdd(&tickets[tile], 1) == Sx - 1);
+        __syncthreads();
+        if (s_last) {
+            __threadfence();
+            const int n = tile * TILE_COLS + 4 * tid;  // 4 columns per thread
+            if (n < N) {
+#pragma unroll
+                for (int t = 0; t < T; ++t) {
+                    float4 a = make_float4(0.f, 0.f, 0.f, 0.f);
+                    for (int s = 0; s < Sx; ++s) {
+                        const float4 v = __ldcg(reinterpret_cast<const float4*>(part + ((size_t)s * T + t) * N + n));
+                        a.x += v.x; a.y += v.y; a.z += v.z; a.w += v.w;
+                    }
+                    *reinterpret_cast<float4*>(y + (size_t)t * N + n) = a;
+                }
+            }
+            if (tid == 0) tickets[tile] = 0;  // ready for the next launch on this workspace
+        }
+    }
 }
 
-// y[t][n] = sum_{s=0}^{S-1} part[s][t][n], always in the same order: warp w adds s = w, w+8, ...
-// sequentially, then the 8 warp sums are added in order w = 0..7.
+// y[t][n] = sum_{s=0}^{S-1} part[s][t][n], sequentially in s: the same order as the fused second pass, so the
+// two-launch form returns the same bits.
 __global__ void __launch_bounds__(VTHREADS)
 vmm_reduce_kernel(const float* __restrict__ part, int S, int T, int N, float* __restrict__ y) {
-    __shared__ float4 red[VW][32];
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int t = blockIdx.y;
-    const int n = blockIdx.x * 128 + lane * 4;
+    const int n = (blockIdx.x * VTHREADS + threadIdx.x) * 4;
+    if (n >= N) return;
     float4 a = make_float4(0.f, 0.f, 0.f, 0.f);
-    if (n < N) {
-        for (int s = warp; s < S; s += VW) {
-            const float4 v = *reinterpret_cast<const float4*>(part + ((size_t)s * T + t) * N + n);
-            a.x += v.x; a.y += v.y; a.z += v.z; a.w += v.w;
-        }
+    for (int s = 0; s < S; ++s) {
+        const float4 v = *reinterpret_cast<const float4*>(part + ((size_t)s * T + t) * N + n);
+        a.x += v.x; a.y += v.y; a.z += v.z; a.w += v.w;
     }
-    red[warp][lane] = a;
-    __syncthreads();
-    if (warp == 0 && n < N) {
-        float4 r = red[0][lane];
-#pragma unroll
-        for (int w = 1; w < VW; ++w) {
-            const float4 v = red[w][lane];
-            r.x += v.x; r.y += v.y; r.z += v.z; r.w += v.w;
-        }
-        *reinterpret_cast<float4*>(y + (size_t)t * N + n) = r;
-    }
+    *reinterpret_cast<float4*>(y + (size_t)t * N + n) = a;
 }
 
-template <int T, bool A16>
+constexpr size_t TICKET_BYTES = 16384;  // head of the workspace: one int per column tile, zero between launches
+
+template <int T, bool A16, bool FUSED>
 static int launch_main_impl(int K, int N, const VmmPlan& pl, const uint32_t* planes, const void* scales,
-                            const void* zeros, const uint32_t* gsched, const uint8_t* gcnt_ge, float* part,
-                            cudaStream_t st) {
+                            const void* zeros, const uint32_t* gsched, const uint8_t* gcnt_ge, void* workspace,
+                            float* y, cudaStream_t st) {
     constexpr int smem = Cfg<T>::SMEM;
     static bool configured = false;
     if (!configured) {
-        if (cudaFuncSetAttribute(vmm_main_kernel<T, A16>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) !=
+        if (cudaFuncSetAttribute(vmm_main_kernel<T, A16, FUSED>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) !=
             cudaSuccess)
             return GRINQH_ERR_CUDA;
         configured = true;
     }
     dim3 grid(pl.col_tiles, pl.Sx);
-    vmm_main_kernel<T, A16><<<grid, VTHREADS, smem, st>>>(K, N, pl.Q, pl.ipw, planes, (const __half*)scales,
-                                                          (const __half*)zeros, gsched, gcnt_ge, part);
+    const uint32_t rq = (65536u + pl.Q - 1) / pl.Q;
+    vmm_main_kernel<T, A16, FUSED><<<grid, VTHREADS, smem, st>>>(
+        K, N, pl.Q, rq, pl.ipw, pl.Sx, planes, (const __half*)scales, (const __half*)zeros, gsched, gcnt_ge,
+        (float*)((char*)workspace + TICKET_BYTES), (int*)workspace, y);
     return cudaGetLastError() == cudaSuccess ? GRINQH_OK : GRINQH_ERR_CUDA;
 }
 
-template <int T>
-static int launch_main(int K, int N, const VmmPlan& pl, const uint32_t* planes, const void* scales,
-                       const void* zeros, const uint32_t* gsched, const uint8_t* gcnt_ge, float* part,
+template <bool FUSED>
+static int launch_main(int T, int K, int N, const VmmPlan& pl, const uint32_t* planes, const void* scales,
+                       const void* zeros, const uint32_t* gsched, const uint8_t* gcnt_ge, void* ws, float* y,
                        cudaStream_t st) {
-    if (N % 128 == 0) return launch_main_impl<T, true>(K, N, pl, planes, scales, zeros, gsched, gcnt_ge, part, st);
-    return launch_main_impl<T, false>(K, N, pl, planes, scales, zeros, gsched, gcnt_ge, part, st);
+#define GQ_LAUNCH(TT)                                                                                              \
+    return (N % 128 == 0)                                                                                          \
+               ? launch_main_impl<TT, true, FUSED>(K, N, pl, planes, scales, zeros, gsched, gcnt_ge, ws, y, st)    \
+               : launch_main_impl<TT, false, FUSED>(K, N, pl, planes, scales, zeros, gsched, gcnt_ge, ws, y, st)
+    switch (T) {
+        case 1: GQ_LAUNCH(1);
+        case 2: GQ_LAUNCH(2);
+        case 3: GQ_LAUNCH(3);
+        default: GQ_LAUNCH(4);
+    }
+#undef GQ_LAUNCH
 }
 
 static int check_vmm_args(int T, int K, int N, int group) {
     if (group != GQ_G || T < 1 || T > GRINQH_MAX_T || K <= 0 || N <= 0 || K % GQ_G || N % 32) return GRINQH_ERR_SHAPE;
+    if ((size_t)((N + TILE_COLS - 1) / TILE_COLS) * sizeof(int) > TICKET_BYTES) return GRINQH_ERR_SHAPE;
+    return GRINQH_OK;
+}
+
+static int check_vmm_ptrs(int T, int K, int N, int group, const void* planes, const void* scales, const void* zeros,
+                          const void* gsched, const void* gcnt_ge, const void* workspace, size_t workspace_bytes) {
+    if (!planes || !scales || !zeros || !gsched || !gcnt_ge || !workspace) return GRINQH_ERR_NULL;
+    const int rc = check_vmm_args(T, K, N, group);
+    if (rc != GRINQH_OK) return rc;
+    if (((uintptr_t)planes | (uintptr_t)scales | (uintptr_t)zeros | (uintptr_t)gsched | (uintptr_t)gcnt_ge |
+         (uintptr_t)workspace) & 15)
+        return GRINQH_ERR_ALIGN;
+    if (workspace_bytes < grinqh_vmm_workspace_bytes(T, K, N)) return GRINQH_ERR_WORKSPACE;
     return GRINQH_OK;
 }
 
@@ -412,28 +452,37 @@ static int check_vmm_args(int T, int K, int N, int group) {
 extern "C" size_t grinqh_vmm_workspace_bytes(int T, int K, int N) {
     if (gq::check_vmm_args(T, K, N, GQ_G) != GRINQH_OK) return 0;
     const gq::VmmPlan pl = gq::vmm_plan(T, K, N);
-    return (size_t)pl.Sx * T * N * sizeof(float);
+    return gq::TICKET_BYTES + (size_t)pl.Sx * T * N * sizeof(float);
+}
+
+extern "C" int grinqh_vmm_workspace_init(void* workspace, size_t workspace_bytes, void* stream) {
+    if (!workspace) return GRINQH_ERR_NULL;
+    if ((uintptr_t)workspace & 15) return GRINQH_ERR_ALIGN;
+    if (workspace_bytes < gq::TICKET_BYTES) return GRINQH_ERR_WORKSPACE;
+    return cudaMemsetAsync(workspace, 0, gq::TICKET_BYTES, (cudaStream_t)stream) == cudaSuccess ? GRINQH_OK
+                                                                                                : GRINQH_ERR_CUDA;
+}
+
+extern "C" int grinqh_vmm(int T, int K, int N, int group, const uint32_t* planes, const void* scales_f16,
+                          const void* zeros_f16, const uint32_t* gsched, const uint8_t* gcnt_ge, float* y,
+                          void* workspace, size_t workspace_bytes, void* stream) {
+    if (!y) return GRINQH_ERR_NULL;
+    if ((uintptr_t)y & 15) return GRINQH_ERR_ALIGN;
+    const int rc = gq::check_vmm_ptrs(T, K, N, group, planes, scales_f16, zeros_f16, gsched, gcnt_ge, workspace,
+                                      workspace_bytes);
+    if (rc != GRINQH_OK) return rc;
+    return gq::launch_main<true>(T, K, N, gq::vmm_plan(T, K, N), planes, scales_f16, zeros_f16, gsched, gcnt_ge,
+                                 workspace, y, (cudaStream_t)stream);
 }
 
 extern "C" int grinqh_vmm_main(int T, int K, int N, int group, const uint32_t* planes, const void* scales_f16,
                                const void* zeros_f16, const uint32_t* gsched, const uint8_t* gcnt_ge,
                                void* workspace, size_t workspace_bytes, void* stream) {
-    if (!planes || !scales_f16 || !zeros_f16 || !gsched || !gcnt_ge || !workspace) return GRINQH_ERR_NULL;
-    int rc = gq::check_vmm_args(T, K, N, group);
+    const int rc = gq::check_vmm_ptrs(T, K, N, group, planes, scales_f16, zeros_f16, gsched, gcnt_ge, workspace,
+                                      workspace_bytes);
     if (rc != GRINQH_OK) return rc;
-    if (((uintptr_t)planes | (uintptr_t)scales_f16 | (uintptr_t)zeros_f16 | (uintptr_t)gsched |
-         (uintptr_t)gcnt_ge | (uintptr_t)workspace) & 15)
-        return GRINQH_ERR_ALIGN;
-    if (workspace_bytes < grinqh_vmm_workspace_bytes(T, K, N)) return GRINQH_ERR_WORKSPACE;
-    const gq::VmmPlan pl = gq::vmm_plan(T, K, N);
-    cudaStream_t st = (cudaStream_t)stream;
-    float* part = (float*)workspace;
-    switch (T) {
-        case 1: return gq::launch_main<1>(K, N, pl, planes, scales_f16, zeros_f16, gsched, gcnt_ge, part, st);
-        case 2: return gq::launch_main<2>(K, N, pl, planes, scales_f16, zeros_f16, gsched, gcnt_ge, part, st);
-        case 3: return gq::launch_main<3>(K, N, pl, planes, scales_f16, zeros_f16, gsched, gcnt_ge, part, st);
-        default: return gq::launch_main<4>(K, N, pl, planes, scales_f16, zeros_f16, gsched, gcnt_ge, part, st);
-    }
+    return gq::launch_main<false>(T, K, N, gq::vmm_plan(T, K, N), planes, scales_f16, zeros_f16, gsched, gcnt_ge,
+                                  workspace, nullptr, (cudaStream_t)stream);
 }
 
 extern "C" int grinqh_vmm_reduce(int T, int K, int N, float* y, const void* workspace, size_t workspace_bytes,
@@ -444,18 +493,8 @@ extern "C" int grinqh_vmm_reduce(int T, int K, int N, float* y, const void* work
     if (((uintptr_t)y | (uintptr_t)workspace) & 15) return GRINQH_ERR_ALIGN;
     if (workspace_bytes < grinqh_vmm_workspace_bytes(T, K, N)) return GRINQH_ERR_WORKSPACE;
     const gq::VmmPlan pl = gq::vmm_plan(T, K, N);
-    dim3 grid((N + 127) / 128, T);
-    gq::vmm_reduce_kernel<<<grid, gq::VTHREADS, 0, (cudaStream_t)stream>>>((const float*)workspace, pl.Sx, T, N, y);
+    dim3 grid((N + 4 * gq::VTHREADS - 1) / (4 * gq::VTHREADS), T);
+    gq::vmm_reduce_kernel<<<grid, gq::VTHREADS, 0, (cudaStream_t)stream>>>(
+        (const float*)((const char*)workspace + gq::TICKET_BYTES), pl.Sx, T, N, y);
     return cudaGetLastError() == cudaSuccess ? GRINQH_OK : GRINQH_ERR_CUDA;
-}
-
-extern "C" int grinqh_vmm(int T, int K, int N, int group, const uint32_t* planes, const void* scales_f16,
-                          const void* zeros_f16, const uint32_t* gsched, const uint8_t* gcnt_ge, float* y,
-                          void* workspace, size_t workspace_bytes, void* stream) {
-    if (!y) return GRINQH_ERR_NULL;
-    if ((uintptr_t)y & 15) return GRINQH_ERR_ALIGN;
-    int rc = grinqh_vmm_main(T, K, N, group, planes, scales_f16, zeros_f16, gsched, gcnt_ge, workspace,
-                             workspace_bytes, stream);
-    if (rc != GRINQH_OK) return rc;
-    return grinqh_vmm_reduce(T, K, N, y, workspace, workspace_bytes, stream);
 }

@@ -47,6 +47,12 @@ LLAMA3_8B_LAYER = (
 LLAMA3_8B_INPUTS = {"q": "attn_in", "k": "attn_in", "v": "attn_in", "o": "o_in",
                     "gate": "mlp_in", "up": "mlp_in", "down": "down_in"}
 LLAMA3_8B_INPUT_DIMS = {"attn_in": 4096, "o_in": 4096, "mlp_in": 4096, "down_in": 14336}
+# launch plan of the same layer with same-input projections concatenated along N (the quantiser is per column, so
+# packing [W_q | W_k | W_v] equals concatenating the three packs): 4 VMM launches instead of 7
+LLAMA3_8B_LAYER_FUSED = (
+    ("qkv", 4096, 4096 + 1024 + 1024, "attn_in"), ("o", 4096, 4096, "o_in"),
+    ("gate_up", 4096, 2 * 14336, "mlp_in"), ("down", 14336, 4096, "down_in"),
+)
 QWEN3_8B_SHAPES = ((4096, 4096), (4096, 1024), (4096, 12288), (12288, 4096))
 LLAMA3_70B_SHAPES = ((8192, 8192), (8192, 1024), (8192, 28672), (28672, 8192))
 

@@ -228,7 +228,27 @@ def test_decode_host_entry(gq):
     yh = torch.empty((1, N), dtype=torch.float32).pin_memory()
     xd = torch.empty((1, K), dtype=torch.float16, device="cuda")
     yd = torch.empty((1, N), dtype=torch.float32, device="cuda")
-    ws = torch.empty((gq.grinqh_vmm_workspace_bytes(1, K, N),), dtype=torch.uint8, device="cuda")
+    ws = gq.grinqh_vmm_workspace(1, K, N)
     gq.grinqh_decode_host(xh, counts, w, a, xd, yd, ws, yh)
     torch.cuda.synchronize()
     assert rel_l2(yh.numpy(), y_ref) <= TOL
+
+
+def test_fused_second_pass_matches_two_launches_and_workspace_is_reusable(gq):
+    """grinqh_vmm (last CTA per tile reduces) == grinqh_vmm_main + grinqh_vmm_reduce bit for bit, repeatedly and
+    across shapes sharing one workspace (the tickets must come back to zero after every launch)."""
+    shapes = [(1, 1024, 2048), (2, 512, 4096 + 96), (1, 2048, 1024), (4, 256, 512)]
+    ws = gq.grinqh_vmm_workspace(4, 2048, 4096 + 96)
+    packed = {}
+    for rep in range(3):
+        for T, K, N in shapes:
+            if (K, N) not in packed:
+                packed[(K, N)] = gq.grinqh_pack(_dev(synth.make_weights(K, N, 0.02, K + N)))
+            w = packed[(K, N)]
+            x = synth.make_x(T, K, 100 + rep, "student_t")
+            a = gq.grinqh_assign(_dev(x), oracle.mix_to_counts(K, synth.MIXES["4"]))
+            y1 = gq.grinqh_vmm(w, a, workspace=ws).cpu().numpy()
+            gq.grinqh_vmm_main(w, a, ws)
+            y2 = torch.empty((T, N), dtype=torch.float32, device="cuda")
+            gq.grinqh_vmm_reduce(T, K, N, y2, ws)
+            assert np.array_equal(y1, y2.cpu().numpy())
