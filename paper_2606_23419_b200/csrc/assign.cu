@@ -98,6 +98,9 @@ assign_kernel(const uint16_t* __restrict__ x, AssignParams p, uint8_t* __restric
         for (int i = 0; i < CNT_BYTES / 16 / AT; ++i) z[tid + i * AT] = make_uint4(0, 0, 0, 0);
     };
 
+    pdl_launch_dependents();
+    pdl_wait();  // x may come from the previous kernel; the outputs may still be read by it
+
     for (int t = 0; t < p.T; ++t) {
         // ---- load the token's local groups (raw patterns; the key is pattern & 0x7FFF)
         for (int i = tid; i < nloc * (GQ_G / 4); i += AT)
@@ -396,7 +399,8 @@ extern "C" int grinqh_assign(const void* x_f16, int T, int K, const uint32_t cou
             return GRINQH_ERR_CUDA;
         configured = true;
     }
-    gq::assign_kernel<<<gq::NC, gq::AT, smem, (cudaStream_t)stream>>>((const uint16_t*)x_f16, p, bits, bits_union, rows,
-                                                                cnt_ge, grows, gcnt_ge, gsched);
-    return cudaGetLastError() == cudaSuccess ? GRINQH_OK : GRINQH_ERR_CUDA;
+    const cudaError_t e = gq::launch_pdl(gq::assign_kernel, dim3(gq::NC), dim3(gq::AT), smem, (cudaStream_t)stream,
+                                         (const uint16_t*)x_f16, p, bits, bits_union, rows, cnt_ge, grows, gcnt_ge,
+                                         gsched);
+    return e == cudaSuccess ? GRINQH_OK : GRINQH_ERR_CUDA;
 }

@@ -36,4 +36,27 @@ __device__ __forceinline__ void fhfma_hi(float& acc, uint32_t a, uint16_t x) {
         : "+f"(acc) : "r"(a), "h"(x));
 }
 
+// Programmatic dependent launch (PDL): every per-step kernel is launched with programmatic stream serialization,
+// calls pdl_launch_dependents() at its top (the next kernel of the stream may be scheduled as SMs free up) and
+// pdl_wait() before its first global-memory access (blocks until the previous kernel has completed and flushed).
+// Launch latency, CTA scheduling and the prologue arithmetic of kernel n+1 overlap the tail of kernel n.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
+template <typename... KArgs, typename... Args>
+static inline cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st,
+                                     Args... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+}
+
 }  // namespace gq

@@ -147,6 +147,9 @@ vmm_main_kernel(int K, int N, int Q, uint32_t rq, int ipw, int Sx, const uint32_
                               (A16 ? (size_t)pj * pbytes + (size_t)(tile * 32 + seg * 4) * 4 : (size_t)word * 4);
     const uint32_t lane_dst = A16 ? ring_s + pj * 128 + seg * 16 : ring_s + lane * 4;
 
+    pdl_launch_dependents();
+    pdl_wait();  // nothing global (schedule, partials, tickets) is touched before the previous kernel has finished
+
     const int ws = sx * VW + warp;
     const int it0 = ws * ipw;
     const int it1 = min(I, it0 + ipw);
@@ -406,10 +409,10 @@ static int launch_main_impl(int K, int N, const VmmPlan& pl, const uint32_t* pla
     }
     dim3 grid(pl.col_tiles, pl.Sx);
     const uint32_t rq = (65536u + pl.Q - 1) / pl.Q;
-    vmm_main_kernel<T, A16, FUSED><<<grid, VTHREADS, smem, st>>>(
-        K, N, pl.Q, rq, pl.ipw, pl.Sx, planes, (const __half*)scales, (const __half*)zeros, gsched, gcnt_ge,
-        (float*)((char*)workspace + TICKET_BYTES), (int*)workspace, y);
-    return cudaGetLastError() == cudaSuccess ? GRINQH_OK : GRINQH_ERR_CUDA;
+    const cudaError_t e = launch_pdl(vmm_main_kernel<T, A16, FUSED>, grid, dim3(VTHREADS), (size_t)smem, st, K, N, pl.Q, rq,
+                                     pl.ipw, pl.Sx, planes, (const __half*)scales, (const __half*)zeros, gsched,
+                                     gcnt_ge, (float*)((char*)workspace + TICKET_BYTES), (int*)workspace, y);
+    return e == cudaSuccess ? GRINQH_OK : GRINQH_ERR_CUDA;
 }
 
 template <bool FUSED>
