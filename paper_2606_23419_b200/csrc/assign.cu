@@ -6,12 +6,13 @@
 // them per lane; ballot-matching inside a warp costs as much in issue slots).  Counting is THREAD-PRIVATE instead:
 // thread t owns byte column t of cnt[slot][digit][512], so a histogram update is a plain LDS/ADD/STS with no
 // conflicts; a row is summed afterwards with dp4a, the 8 CTAs' row sums are read through DSMEM and every CTA
-// takes the same decisions on its own copy (no central CTA, one cluster barrier per level).
-// Per token a radix select on the 15-bit fp16 magnitude, 3 + 4 + 4 + 4 bits from the top: every distinct cut
+// takes the same decisions on its own copy (no central CTA, one cluster barrier per level, 3 levels).
+// Per token a radix select on the 15-bit fp16 magnitude, 5 + 5 + 5 bits from the top: every distinct cut
 // C_d keeps (prefix, rank still needed inside the prefix); cuts with the same prefix share a histogram slot.
 // After the last level thr_d is the exact cut key, take_d how many of the keys equal to thr_d are inside, and
 // the cut "splits" if take_d is smaller than their number (ties go to the lower index): only then an ordered
-// count of the equal keys (per 128-row group, then a scan over groups) decides them.  fp16 has few distinct
+// count of the equal keys decides them (lower-ranked CTAs: known from the last level's row sums; inside a CTA:
+// per 128-row group, then a scan over its groups — no extra cluster barrier).  fp16 has few distinct
 // magnitudes, so splits are the common case, not the exception.
 // Widths: b = sum_d mult_d [key above cut d].  Lists: one warp per 128-row group partitions its rows by
 // (width desc, index asc) with ballots -> grows, gcnt_ge, gsched; a scan over the groups' per-width counts
@@ -27,7 +28,7 @@ namespace gq {
 constexpr int AT = 512;   // threads per CTA
 constexpr int AWARPS = AT / 32;
 constexpr int MAXG = GQ_MAX_K / GQ_G;     // 256 groups
-constexpr int CNT_BYTES = 8 * 16 * AT;    // cnt[8 slots][16 digits][1024 thread columns] u8
+constexpr int CNT_BYTES = 8 * 32 * AT;    // cnt[8 slots][32 digits][512 thread columns] u8 = 128 KB
 
 struct AssignParams {
     int T, K;
@@ -68,7 +69,9 @@ __device__ __forceinline__ void scan_groups(uint16_t (*tab)[10], int col, int gr
 }
 
 constexpr int NC = 8;             // CTAs in the cluster (portable maximum); CTA r owns a contiguous run of groups
-constexpr int MAXLG = MAXG / NC;  // groups per CTA
+constexpr int MAXLG = MAXG / NC;  // groups per CTA (32: one per lane in the local scans)
+constexpr int NLEVEL = 3;         // 5 + 5 + 5 bits of the 15-bit magnitude
+constexpr int NDIG = 32;          // digits per level = lanes of the locating warp
 
 __global__ void __cluster_dims__(NC, 1, 1) __launch_bounds__(AT, 1)
 assign_kernel(const uint16_t* __restrict__ x, AssignParams p, uint8_t* __restrict__ bits,
@@ -76,14 +79,14 @@ assign_kernel(const uint16_t* __restrict__ x, AssignParams p, uint8_t* __restric
               uint8_t* __restrict__ grows, uint8_t* __restrict__ gcnt_ge, uint32_t* __restrict__ gsched) {
     cg::cluster_group cluster = cg::this_cluster();
     const int rank = (int)cluster.block_rank();
-    extern __shared__ __align__(16) uint8_t cnt[];                  // [8][16][AT] u8 thread-private counters
+    extern __shared__ __align__(16) uint8_t cnt[];                  // [8 slots][32 digits][AT] u8 thread-private counters
     __shared__ __align__(16) uint16_t xs[MAXLG * GQ_G];             // raw fp16 patterns, local groups, current token
     __shared__ __align__(16) uint8_t glist[MAXLG * GQ_G];
     __shared__ __align__(16) uint8_t gcs[MAXLG][GQ_GCNT];
-    __shared__ uint16_t tab[MAXG][10];                              // replicated: every CTA holds all groups
-    __shared__ int s_rowL[4][8 * 16];                               // this CTA's row sums, one array per level
-    __shared__ int s_row[8 * 16];                                   // cluster-wide row sums of the current level
-    __shared__ int s_pre[8], s_need[8], s_h[8], s_tot[10];
+    __shared__ uint16_t tab[MAXG][10];                              // replicated: per-width counts of every group
+    __shared__ uint16_t ltab[MAXLG][8];                             // local groups: equal-key counts per cut
+    __shared__ int s_rowL[NLEVEL][8 * NDIG];                        // this CTA's row sums, one array per level
+    __shared__ int s_pre[8], s_need[8], s_h[8], s_lead[8], s_slot[8], s_tiebase[8], s_tot[10];
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int K = p.K, groups = K / GQ_G, nd = p.nd;
@@ -92,10 +95,9 @@ assign_kernel(const uint16_t* __restrict__ x, AssignParams p, uint8_t* __restric
     const int nloc = max(0, min(gpc, groups - gl0));
     const uint32_t lt_mask = (1u << lane) - 1u;
 
-    auto zero_cnt = [&]() {
+    auto zero_cnt = [&]() {  // only the rows a level can touch
         uint4* z = reinterpret_cast<uint4*>(cnt);
-#pragma unroll
-        for (int i = 0; i < CNT_BYTES / 16 / AT; ++i) z[tid + i * AT] = make_uint4(0, 0, 0, 0);
+        for (int i = tid; i < nd * NDIG * AT / 16; i += AT) z[i] = make_uint4(0, 0, 0, 0);
     };
 
     pdl_launch_dependents();
@@ -110,40 +112,32 @@ assign_kernel(const uint16_t* __restrict__ x, AssignParams p, uint8_t* __restric
             s_pre[tid] = 0;
             s_need[tid] = (tid < nd) ? p.Cd[tid] : 0;
             s_h[tid] = 0;
+            s_lead[tid] = (tid == 0);  // level 0: one empty prefix, one slot
+            s_slot[tid] = 0;
+            s_tiebase[tid] = 0;
         }
         __syncthreads();
 
-        // ---- radix select, 3 + 4 + 4 + 4 bits
+        // ---- radix select, 5 + 5 + 5 bits: every distinct cut keeps (prefix, rank still needed inside it)
 #pragma unroll 1
-        for (int level = 0; level < 4; ++level) {
-            const int nb = level ? 4 : 3;
-            const int sh = 12 - 4 * level;
-            int pre[8], slot[8];
-#pragma unroll
-            for (int d = 0; d < 8; ++d) pre[d] = (d < nd) ? s_pre[d] : -1 - d;
-#pragma unroll
-            for (int d = 0; d < 8; ++d) {
-                slot[d] = d;
-#pragma unroll
-                for (int e = d - 1; e >= 0; --e)
-                    if (pre[e] == pre[d]) slot[d] = e;
-            }
-            // pass: count the digit of every local key whose prefix is a live one, in this thread's own columns
+        for (int level = 0; level < NLEVEL; ++level) {
+            const int sh = 10 - 5 * level;
+            // pass: count the digit of every local key whose prefix is live, in this thread's own byte columns
             for (int i = tid; i < nloc * GQ_G; i += AT) {
                 const uint32_t m = xs[i] & 0x7FFFu;
-                const int pe = (int)(m >> (sh + nb));
+                const int pe = (int)(m >> (sh + 5));
                 int s = -1;
-#pragma unroll
-                for (int d = 7; d >= 0; --d)
-                    if (slot[d] == d && pe == pre[d]) s = d;
+                for (int d = 0; d < nd; ++d)
+                    if (s_lead[d] && s_pre[d] == pe) s = d;
                 if (s >= 0) {
-                    uint8_t* c = cnt + ((s * 16 + (int)((m >> sh) & ((1u << nb) - 1u))) * AT + tid);
+                    uint8_t* c = cnt + ((s * NDIG + (int)((m >> sh) & 31u)) * AT + tid);
                     *c = (uint8_t)(*c + 1);
                 }
             }
             __syncthreads();
-            // reduce: a warp sums one row (AT bytes) of the live slots
-            for (int r = warp; r < nd * 16; r += AWARPS) {
+            // reduce: a warp sums one row (AT bytes) of a live slot
+            for (int r = warp; r < nd * NDIG; r += AWARPS) {
+                if (!s_lead[r / NDIG]) continue;
                 const uint4 a = reinterpret_cast<const uint4*>(cnt + r * AT)[lane];
                 uint32_t s = 0;
                 s = __dp4a(a.x, 0x01010101u, s); s = __dp4a(a.y, 0x01010101u, s);
@@ -152,33 +146,40 @@ assign_kernel(const uint16_t* __restrict__ x, AssignParams p, uint8_t* __restric
                 if (lane == 0) s_rowL[level][r] = (int)s;
             }
             cluster.sync();
-            // gather the 8 CTAs' row sums (DSMEM), then every CTA takes the same decisions on its own copy
-            if (tid < nd * 16) {
-                int s = 0;
-#pragma unroll
-                for (int r = 0; r < NC; ++r) s += cluster.map_shared_rank(&s_rowL[0][0], r)[level * 128 + tid];
-                s_row[tid] = s;
-            }
-            if (level < 3) zero_cnt();
-            __syncthreads();
+            // locate: warp d reads the 8 CTAs' sums of its slot's 32 digits (DSMEM) and scans them from the top;
+            // every CTA takes the same decision on its own copy
             if (warp < nd) {
-                const int d = warp;
-                int sl = 0;
+                const int d = warp, digit = NDIG - 1 - lane;
+                const int idx = level * (8 * NDIG) + s_slot[d] * NDIG + digit;
+                int h = 0, mine_below = 0;
 #pragma unroll
-                for (int e = 0; e < 8; ++e)
-                    if (e == d) sl = slot[e];
-                const int digit = (1 << nb) - 1 - lane;
-                const int h = (digit >= 0) ? s_row[sl * 16 + digit] : 0;
+                for (int r = 0; r < NC; ++r) {
+                    const int v = cluster.map_shared_rank(&s_rowL[0][0], r)[idx];
+                    h += v;
+                    if (r < rank) mine_below += v;
+                }
                 const int incl = warp_incl_scan(h, lane);
                 const int above = incl - h, need = s_need[d], pr = s_pre[d];
                 __syncwarp();
                 if (above < need && need <= above + h) {
-                    s_pre[d] = (pr << nb) | digit;
+                    s_pre[d] = (pr << 5) | digit;
                     s_need[d] = need - above;
                     s_h[d] = h;
+                    s_tiebase[d] = mine_below;  // after the last level: keys equal to the cut in lower-ranked CTAs
                 }
             }
             __syncthreads();
+            if (level + 1 < NLEVEL) {
+                if (tid < 8) {  // slots of the next level: cuts with the same prefix share one
+                    int sl = tid;
+                    for (int e = tid - 1; e >= 0; --e)
+                        if (s_pre[e] == s_pre[tid]) sl = e;
+                    s_slot[tid] = sl;
+                    s_lead[tid] = (tid < nd && sl == tid);
+                }
+                zero_cnt();
+                __syncthreads();
+            }
         }
         int thr[8], take[8], mult[8];
         bool split[8], anysplit = false;
@@ -190,9 +191,10 @@ assign_kernel(const uint16_t* __restrict__ x, AssignParams p, uint8_t* __restric
             split[d] = (d < nd) && take[d] < s_h[d];
             anysplit |= split[d];
         }
-        if (anysplit) {  // cluster-uniform
-            // ---- a cut splits a run of equal keys: ordered (index-ascending) count of the equal keys;
-            //      every CTA gets every group's count (remote stores), then scans its own copy
+        if (anysplit) {  // cluster-uniform, but everything in here is CTA-local
+            // ---- a cut splits a run of equal keys: ordered (index-ascending) count of the equal keys.  Keys equal
+            //      to the cut in lower-ranked CTAs are already known (s_tiebase, from the last level's row sums);
+            //      inside the CTA: count per local group, then a scan over the (at most 32) local groups.
             for (int lg = warp; lg < nloc; lg += AWARPS) {
                 const uint2 kv = *reinterpret_cast<const uint2*>(xs + lg * GQ_G + 4 * lane);
                 const int m[4] = {(int)(kv.x & 0x7FFF), (int)((kv.x >> 16) & 0x7FFF), (int)(kv.y & 0x7FFF),
@@ -205,18 +207,15 @@ assign_kernel(const uint16_t* __restrict__ x, AssignParams p, uint8_t* __restric
 #pragma unroll
                         for (int i = 0; i < 4; ++i) c += (m[i] == thr[d]);
                         c = __reduce_add_sync(0xffffffffu, c);
-                        if ((lane & 7) == d) mine = c;
+                        if (lane == d) mine = c;
                     }
-                // lane = 8 * r' + d (r' < 4) stores column d to CTAs r' and r' + 4
-                if (split[lane & 7]) {
-                    cluster.map_shared_rank(&tab[0][0], lane >> 3)[(gl0 + lg) * 10 + (lane & 7)] = (uint16_t)mine;
-                    cluster.map_shared_rank(&tab[0][0], (lane >> 3) + 4)[(gl0 + lg) * 10 + (lane & 7)] = (uint16_t)mine;
-                }
+                if (lane < 8) ltab[lg][lane] = (uint16_t)mine;
             }
-            cluster.sync();
-            if (warp < 8 && split[warp]) {
-                int dummy;
-                scan_groups(tab, warp, groups, lane, &dummy);
+            __syncthreads();
+            if (warp < 8 && split[warp]) {  // lane = local group
+                const int v = (lane < nloc) ? ltab[lane][warp] : 0;
+                const int excl = warp_incl_scan(v, lane) - v;
+                if (lane < nloc) ltab[lane][warp] = (uint16_t)(excl + s_tiebase[warp]);
             }
             __syncthreads();
         }
@@ -234,7 +233,7 @@ assign_kernel(const uint16_t* __restrict__ x, AssignParams p, uint8_t* __restric
                     for (int i = 0; i < 4; ++i) b[i] += (m[i] >= thr[d]) ? mult[d] : 0;
                 } else {
                     bool eq[4];
-                    int below = tab[g][d];  // equal keys in earlier groups
+                    int below = ltab[lg][d];  // equal keys at lower indices outside this group
 #pragma unroll
                     for (int i = 0; i < 4; ++i) {
                         eq[i] = (m[i] == thr[d]);
@@ -253,9 +252,7 @@ assign_kernel(const uint16_t* __restrict__ x, AssignParams p, uint8_t* __restric
             if (t == 0) *u = packed;
             else *u = __vmaxu4(*u, packed);
         }
-        // tab is rewritten remotely by the next token / the width counts: everybody must be done reading it
-        if (anysplit) cluster.sync();
-        else __syncthreads();
+        __syncthreads();
     }
 
     // ---- per-group lists of the local groups
