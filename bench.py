@@ -173,6 +173,17 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+def max_over_ranks(values, device=None):
+    """Replicas only: the ranks share nothing on the data path; the job's time is the slowest rank's."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return [float(v) for v in values]
+    t = torch.tensor([float(v) for v in values], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(v) for v in t.tolist()]
+
+
 # ------------------------------------------------------------------------------------------ native arm
 def run_native(args):
     import numpy as np
@@ -319,11 +330,7 @@ def run_native(args):
                 g_split[i % L].replay()
             ms_split = timed(g_split, args.steps)
 
-    if world > 1:
-        import torch.distributed as dist
-        t = torch.tensor([ms_total, ms_main, ms_host, ms_split or 0.0], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total, ms_main, ms_host, ms_split = [float(v) for v in t.tolist()]
+    ms_total, ms_main, ms_host, ms_split = max_over_ranks([ms_total, ms_main, ms_host, ms_split or 0.0], dev)
 
     # ---- algorithmic bytes of the VMM launches of one step (measured widths; SURVEY.md 8d / DESIGN.md)
     step_bytes, plane_bytes = 0, 0

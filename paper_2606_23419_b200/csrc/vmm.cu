@@ -163,6 +163,14 @@ vmm_main_kernel(int K, int N, int Q, uint32_t rq, int ipw, int Sx, const uint32_
         auto rows_ge = [&](uint32_t c) -> int {  // rows of this item among the first c list positions
             return ((int)c > q) ? (int)(((c - q + Q - 1) * rq) >> 16) : 0;
         };
+        // the schedule entries are fetched speculatively (position < 128), in flight together with the counts
+        uint32_t ev[T][4];
+#pragma unroll
+        for (int jj = 0; jj < 4; ++jj) {
+            const int pos = q + (lane + 32 * jj) * Q;
+#pragma unroll
+            for (int t = 0; t < T; ++t) ev[t][jj] = (pos < GQ_G) ? gsched[(size_t)t * K + g * GQ_G + pos] : 0u;
+        }
         const int n_rows = rows_ge((cv.x >> 8) & 0xFF);
         float X[T], Phi[T];
 #pragma unroll
@@ -171,16 +179,12 @@ vmm_main_kernel(int K, int N, int Q, uint32_t rq, int ipw, int Sx, const uint32_
         for (int jj = 0; jj < 4; ++jj) {
             const int i = lane + 32 * jj;
             if (i < n_rows) {
-                const int p = g * GQ_G + q + i * Q;
-                const uint32_t e0 = gsched[p];
+                const uint32_t e0 = ev[0][jj];
                 s_item[i] = make_uint2(e0, (e0 & 0xFFu) * rowbytes);
 #pragma unroll
                 for (int t = 0; t < T; ++t) {
-                    uint32_t e = e0;
-                    if (t > 0) {
-                        e = gsched[(size_t)t * K + p];
-                        s_tok[(t - 1) * GQ_G + i] = e;
-                    }
+                    const uint32_t e = ev[t][jj];
+                    if (t > 0) s_tok[(t - 1) * GQ_G + i] = e;
                     const int bt = (e >> 8) & 15;
                     if (bt > 0) {
                         const float xf = __half2float(__ushort_as_half((uint16_t)(e >> 16)));
@@ -225,6 +229,17 @@ vmm_main_kernel(int K, int N, int Q, uint32_t rq, int ipw, int Sx, const uint32_
         using HiT = std::integral_constant<bool, true>;
         using LoT = std::integral_constant<bool, false>;
 
+        // The group's scales and zeros (64 B + 64 B per lane) ride the ring too: chunk c = the lane's 16-byte piece c
+        // of both, copied into the slot that frees up at iteration first_i + c (no row left to prefetch there), so
+        // the item-end arithmetic never waits on a fresh global load.  chunk c <-> slot (first_i + c - 1) mod RING.
+        const size_t gn = (size_t)g * N + (size_t)word * 32;
+        const int first_i = max(0, n_rows - (RING - 1));
+        auto issue_sz = [&](int c, uint32_t slot_off) {
+            if (active) {
+                cp_async16(ring_s + slot_off + lane * 16, scales + gn + 8 * c);
+                cp_async16(ring_s + slot_off + 512 + lane * 16, zeros + gn + 8 * c);
+            }
+        };
         uint32_t so = 0;  // ring byte offset of the row being consumed
 #pragma unroll
         for (int i = 0; i < RING - 1; ++i) {
@@ -239,6 +254,7 @@ vmm_main_kernel(int K, int N, int Q, uint32_t rq, int ipw, int Sx, const uint32_
                 cp_async_wait<RING - 2>();
                 __syncwarp();
                 if (i + RING - 1 < n_rows) issue(i + RING - 1, (so - SLOT_BYTES) & RING_MASK, hi_tag);
+                else if (i - first_i < 4) issue_sz(i - first_i, (so - SLOT_BYTES) & RING_MASK);
                 cp_async_commit();
                 const uint32_t m = s_item[i].x;
                 const uint32_t* slot = reinterpret_cast<const uint32_t*>(ring + so) + lane;
@@ -295,17 +311,23 @@ vmm_main_kernel(int K, int N, int Q, uint32_t rq, int ipw, int Sx, const uint32_
             run(integral_constant<int, 2>{}, LoT{}, r3, r2);
             run(integral_constant<int, 0>{}, LoT{}, r2, n_rows);
         }
+        if (n_rows > 0 && n_rows - first_i < 4) {  // chunks that found no free iteration (short items, small rings)
+            __syncwarp();
+            for (int c = n_rows - first_i; c < 4; ++c)
+                issue_sz(c, (uint32_t)((first_i + c - 1) & (RING - 1)) * SLOT_BYTES);
+        }
+        cp_async_commit();
         cp_async_wait<0>();
 
         // ---- item end: s and z once per (item, column), into the warp's accumulator
         if (active) {
-            const size_t gn = (size_t)g * N + (size_t)word * 32;
 #pragma unroll
             for (int L = 0; L < 4; ++L) {
                 float sf[8], zf[8];
                 if (n_rows > 0) {
-                    const uint4 sv = *reinterpret_cast<const uint4*>(scales + gn + 8 * L);
-                    const uint4 zv = *reinterpret_cast<const uint4*>(zeros + gn + 8 * L);
+                    const uint8_t* sz = ring + (uint32_t)((first_i + L - 1) & (RING - 1)) * SLOT_BYTES + lane * 16;
+                    const uint4 sv = *reinterpret_cast<const uint4*>(sz);
+                    const uint4 zv = *reinterpret_cast<const uint4*>(sz + 512);
                     const uint32_t su[4] = {sv.x, sv.y, sv.z, sv.w}, zu[4] = {zv.x, zv.y, zv.z, zv.w};
 #pragma unroll
                     for (int h = 0; h < 4; ++h) {
@@ -366,9 +388,15 @@ vmm_main_kernel(int K, int N, int Q, uint32_t rq, int ipw, int Sx, const uint32_
 #pragma unroll
                 for (int t = 0; t < T; ++t) {
                     float4 a = make_float4(0.f, 0.f, 0.f, 0.f);
-                    for (int s = 0; s < Sx; ++s) {
-                        const float4 v = __ldcg(reinterpret_cast<const float4*>(part + ((size_t)s * T + t) * N + n));
-                        a.x += v.x; a.y += v.y; a.z += v.z; a.w += v.w;
+                    for (int s0 = 0; s0 < Sx; s0 += 16) {  // 16 loads in flight, added in the fixed order
+                        float4 v[16];
+#pragma unroll
+                        for (int j = 0; j < 16; ++j)
+                            if (s0 + j < Sx)
+                                v[j] = __ldcg(reinterpret_cast<const float4*>(part + ((size_t)(s0 + j) * T + t) * N + n));
+#pragma unroll
+                        for (int j = 0; j < 16; ++j)
+                            if (s0 + j < Sx) { a.x += v[j].x; a.y += v[j].y; a.z += v[j].z; a.w += v[j].w; }
                     }
                     *reinterpret_cast<float4*>(y + (size_t)t * N + n) = a;
                 }
