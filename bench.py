@@ -38,6 +38,8 @@ def _args():
     ap.add_argument("--layers", type=int, default=4, help="distinct packed layers the timed loop rotates over")
     ap.add_argument("--seed", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sweep", action="store_true", help="configs 3 and 5: per-VMM latency vs average bits (not the contract line)")
+    ap.add_argument("--decode-step", action="store_true", help="config 4: 32-layer decode step in one CUDA graph")
     ap.add_argument("--no-split", action="store_true", help="skip the one-launch-per-projection variant")
     return ap.parse_args()
 
@@ -388,9 +390,158 @@ def run_native(args):
         dist.destroy_process_group()
 
 
+# ------------------------------------------------------------------------------------------ sweep (not the contract line)
+def run_sweep(args):
+    """BASELINE.json configs 3 and 5: us per VMM and per assign vs average bits, per shape and token count.
+    One JSON line per case on stdout (prefixed "SWEEP "), a linear fit t = a + c * bits per (shape, T)."""
+    import math
+
+    import torch
+
+    from paper_2606_23419_b200 import binding as gq
+    from paper_2606_23419_b200 import synth
+
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    peak, _ = _peaks()
+    gen = torch.Generator(device=dev)
+    gen.manual_seed(args.seed)
+    cases = [("qwen3-8b", K, N, 0.02, "normal", (1,)) for K, N in synth.QWEN3_8B_SHAPES]
+    cases += [("llama3-70b", K, N, 0.015, "student_t", (1, 2, 4)) for K, N in synth.LLAMA3_70B_SHAPES]
+    mixes = ["2", "3", "3.25", "4", "5", "8"]
+    stream = torch.cuda.Stream(device=dev)
+
+    def time_graph(fn, n_inner, reps=20):
+        with torch.cuda.stream(stream):
+            fn()
+            stream.synchronize()
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g, stream=stream):
+                fn()
+            for _ in range(3):
+                g.replay()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            stream.synchronize()
+            a.record(stream)
+            for _ in range(reps):
+                g.replay()
+            b.record(stream)
+            stream.synchronize()
+        return a.elapsed_time(b) * 1e3 / (reps * n_inner)
+
+    for model, K, N, std, dist, Ts in cases:
+        copies = int(math.ceil(300e6 / (K * N))) + 1          # > 2 x L2 of 8-bit codes, rotated
+        packed = []
+        for c in range(copies):
+            W = (torch.randn((K, N), generator=gen, device=dev, dtype=torch.float32) * std).to(torch.float16)
+            packed.append(gq.grinqh_pack(W))
+            del W
+        for T in Ts:
+            ws = gq.grinqh_vmm_workspace(T, K, N, dev)
+            x = torch.from_numpy(synth.make_x(T, K, args.seed + 7, dist)).to(dev)
+            y = torch.empty((T, N), dtype=torch.float32, device=dev)
+            pts = []
+            for mix in mixes:
+                counts = gq.grinqh_mix_to_counts(K, synth.MIXES[mix])
+                a = gq.Assignment(T, K, dev)
+                gq.grinqh_assign(x, counts, a)
+                torch.cuda.synchronize()
+                union_bits = float(a.bits_union.sum().item()) / K
+                us_vmm = time_graph(lambda: [gq.grinqh_vmm(w, a, y, ws) for w in packed], copies)
+                us_asg = time_graph(lambda: [gq.grinqh_assign(x, counts, a) for _ in range(8)], 8)
+                ab = alg_bytes(K, N, T, int(a.bits_union.sum().item()))
+                rec = {"model": model, "K": K, "N": N, "T": T, "mix": mix,
+                       "avg_bits_per_token": synth.mix_avg_bits(synth.MIXES[mix]), "union_bits": union_bits,
+                       "us_vmm": us_vmm, "us_assign": us_asg, "alg_MB": ab / 1e6,
+                       "GBps": ab / us_vmm / 1e3, "frac_of_measured_hbm": ab / us_vmm / 1e3 / peak}
+                pts.append((union_bits, us_vmm))
+                print("SWEEP " + json.dumps(rec), flush=True)
+            n = len(pts)
+            mx, my = sum(p[0] for p in pts) / n, sum(p[1] for p in pts) / n
+            c = sum((p[0] - mx) * (p[1] - my) for p in pts) / sum((p[0] - mx) ** 2 for p in pts)
+            a0 = my - c * mx
+            ss_res = sum((p[1] - (a0 + c * p[0])) ** 2 for p in pts)
+            ss_tot = sum((p[1] - my) ** 2 for p in pts)
+            print("SWEEP " + json.dumps({"model": model, "K": K, "N": N, "T": T, "fit": "us_vmm = a + c * union_bits",
+                                         "a_us": a0, "c_us_per_bit": c, "r2": 1 - ss_res / ss_tot}), flush=True)
+        del packed
+        torch.cuda.empty_cache()
+
+
+# ------------------------------------------------------------------------------------------ 32-layer decode step
+def run_decode_step(args):
+    """BASELINE.json configs[3]: all linear layers of a 32-layer Llama-3-8B-shaped model (6.98 G weights packed to
+    bit planes, ~7 GB), fresh heavy-tailed activations per layer, per-layer rank assignment, ONE CUDA graph of
+    32 x (4 assigns + 4 VMM launches).  One JSON line per mix, prefixed "DECODE "."""
+    import torch
+
+    from paper_2606_23419_b200 import binding as gq
+    from paper_2606_23419_b200 import synth
+
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    peak, _ = _peaks()
+    gen = torch.Generator(device=dev)
+    gen.manual_seed(args.seed)
+    NL, T = 32, 1
+    fused = synth.LLAMA3_8B_LAYER_FUSED
+    in_dims = synth.LLAMA3_8B_INPUT_DIMS
+    packed = []
+    for l in range(NL):
+        d = {}
+        for name, K, N, _ in fused:
+            W = (torch.randn((K, N), generator=gen, device=dev, dtype=torch.float32) * 0.02).to(torch.float16)
+            d[name] = gq.grinqh_pack(W)
+            del W
+        packed.append(d)
+    xs = [{n: torch.from_numpy(synth.make_x(T, K, args.seed + 17 * l + i, "student_t")).to(dev)
+           for i, (n, K) in enumerate(in_dims.items())} for l in range(NL)]
+    assigns = [{n: gq.Assignment(T, K, dev) for n, K in in_dims.items()} for _ in range(NL)]
+    ys = [{name: torch.empty((T, N), dtype=torch.float32, device=dev) for name, K, N, _ in fused} for _ in range(NL)]
+    _, Kw, Nw, _ = max(fused, key=lambda s: gq.grinqh_vmm_workspace_bytes(T, s[1], s[2]))
+    ws = gq.grinqh_vmm_workspace(T, Kw, Nw, dev)
+    stream = torch.cuda.Stream(device=dev)
+    for mix in ("2", "3", "4", "8"):
+        counts = {K: gq.grinqh_mix_to_counts(K, synth.MIXES[mix]) for K in set(in_dims.values())}
+
+        def step():
+            for l in range(NL):
+                for name, K, N, inp in fused:
+                    gq.grinqh_assign(xs[l][inp], counts[K], assigns[l][inp])
+                    gq.grinqh_vmm(packed[l][name], assigns[l][inp], ys[l][name], ws)
+
+        with torch.cuda.stream(stream):
+            step()
+            stream.synchronize()
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g, stream=stream):
+                step()
+            for _ in range(3):
+                g.replay()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            stream.synchronize()
+            reps = 20
+            a.record(stream)
+            for _ in range(reps):
+                g.replay()
+            b.record(stream)
+            stream.synchronize()
+        us = a.elapsed_time(b) * 1e3 / reps
+        nbytes = sum(alg_bytes(K, N, T, int(assigns[l][inp].bits_union.sum().item()))
+                     for l in range(NL) for name, K, N, inp in fused)
+        print("DECODE " + json.dumps({"workload": "32-layer llama3-8b-shaped decode step, 256 launches in one CUDA graph",
+                                      "mix": mix, "avg_bits": synth.mix_avg_bits(synth.MIXES[mix]), "us_per_decode_step": us,
+                                      "alg_GB": nbytes / 1e9, "GBps_incl_assign": nbytes / us / 1e3,
+                                      "frac_of_measured_hbm": nbytes / us / 1e3 / peak}), flush=True)
+
+
 def main():
     args = _args()
-    if args.impl == "reference":
+    if args.decode_step:
+        run_decode_step(args)
+    elif args.sweep:
+        run_sweep(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_native(args)
