@@ -229,75 +229,91 @@ vmm_main_kernel(int K, int N, int Q, uint32_t rq, int ipw, int Sx, const uint32_
         using HiT = std::integral_constant<bool, true>;
         using LoT = std::integral_constant<bool, false>;
 
-        // The group's scales and zeros (64 B + 64 B per lane) ride the ring too: chunk c = the lane's 16-byte piece c
-        // of both, copied into the slot that frees up at iteration first_i + c (no row left to prefetch there), so
-        // the item-end arithmetic never waits on a fresh global load.  chunk c <-> slot (first_i + c - 1) mod RING.
+        // The group's scales and zeros (64 B + 64 B per lane) ride the ring too, as "virtual rows" n_rows .. n_rows+3
+        // behind the item's rows: chunk c = the lane's 16-byte piece c of both.  Virtual row v always lives in slot
+        // v mod RING, and every issue is one cp.async group, so group index == virtual row index.
         const size_t gn = (size_t)g * N + (size_t)word * 32;
-        const int first_i = max(0, n_rows - (RING - 1));
-        auto issue_sz = [&](int c, uint32_t slot_off) {
-            if (active) {
+        int next_v = 0;  // next virtual row to issue
+        auto issue_next = [&](auto hi_tag) {
+            const uint32_t slot_off = (uint32_t)(next_v & (RING - 1)) * SLOT_BYTES;
+            if (next_v < n_rows) {
+                issue(next_v, slot_off, hi_tag);
+            } else if (next_v < n_rows + 4 && active) {
+                const int c = next_v - n_rows;
                 cp_async16(ring_s + slot_off + lane * 16, scales + gn + 8 * c);
                 cp_async16(ring_s + slot_off + 512 + lane * 16, zeros + gn + 8 * c);
             }
-        };
-        uint32_t so = 0;  // ring byte offset of the row being consumed
-#pragma unroll
-        for (int i = 0; i < RING - 1; ++i) {
-            if (i < n_rows) issue(i, i * SLOT_BYTES, HiT{});
             cp_async_commit();
-        }
+            ++next_v;
+        };
+#pragma unroll
+        for (int i = 0; i < RING - 2; ++i) issue_next(HiT{});
 
-        // rows [i0, i1) of the item, all of width B (B = 0: any width, read from the schedule)
-        auto run = [&](auto b_tag, auto hi_tag, int i0, int i1) {
+        // one row: plane words of its ring slot -> 32 truncated codes -> 32 FMAs per token
+        auto consume = [&](auto b_tag, int i) {
             constexpr int B = decltype(b_tag)::value;
-            for (int i = i0; i < i1; ++i) {
-                cp_async_wait<RING - 2>();
-                __syncwarp();
-                if (i + RING - 1 < n_rows) issue(i + RING - 1, (so - SLOT_BYTES) & RING_MASK, hi_tag);
-                else if (i - first_i < 4) issue_sz(i - first_i, (so - SLOT_BYTES) & RING_MASK);
-                cp_async_commit();
-                const uint32_t m = s_item[i].x;
-                const uint32_t* slot = reinterpret_cast<const uint32_t*>(ring + so) + lane;
-                so = (so + SLOT_BYTES) & RING_MASK;
-                uint32_t Wd[8], V[8];
-                if (B == 8) {
+            const uint32_t m = s_item[i].x;
+            const uint32_t* slot = reinterpret_cast<const uint32_t*>(ring + (uint32_t)(i & (RING - 1)) * SLOT_BYTES) + lane;
+            uint32_t Wd[8], V[8];
+            if (B == 8) {
 #pragma unroll
-                    for (int j = 0; j < 8; ++j) Wd[j] = slot[j * 32];
-                    gather<8>(Wd, V);
-                } else if (B == 4) {
+                for (int j = 0; j < 8; ++j) Wd[j] = slot[j * 32];
+                gather<8>(Wd, V);
+            } else if (B == 4) {
 #pragma unroll
-                    for (int j = 0; j < 4; ++j) Wd[j] = slot[j * 32];
-                    gather<4>(Wd, V);
-                } else if (B == 2) {
+                for (int j = 0; j < 4; ++j) Wd[j] = slot[j * 32];
+                gather<4>(Wd, V);
+            } else if (B == 2) {
 #pragma unroll
-                    for (int j = 0; j < 2; ++j) Wd[j] = slot[j * 32];
-                    gather<2>(Wd, V);
-                } else {  // stale slot words beyond the row's planes are masked off
-                    const int b = (m >> 12) & 15;
+                for (int j = 0; j < 2; ++j) Wd[j] = slot[j * 32];
+                gather<2>(Wd, V);
+            } else {  // stale slot words beyond the row's planes are masked off
+                const int b = (m >> 12) & 15;
 #pragma unroll
-                    for (int j = 0; j < 8; ++j) Wd[j] = (j < b) ? slot[j * 32] : 0u;
-                    gather<8>(Wd, V);
-                }
-                if (T == 1) {
-                    accumulate_row(V, (uint16_t)(m >> 16), acc[0]);
-                } else {
-                    const int b = (m >> 12) & 15;
+                for (int j = 0; j < 8; ++j) Wd[j] = (j < b) ? slot[j * 32] : 0u;
+                gather<8>(Wd, V);
+            }
+            if (T == 1) {
+                accumulate_row(V, (uint16_t)(m >> 16), acc[0]);
+            } else {
+                const int b = (m >> 12) & 15;
 #pragma unroll
-                    for (int t = 0; t < T; ++t) {
-                        const uint32_t e = (t == 0) ? m : s_tok[(t - 1) * GQ_G + i];
-                        const int bt = (e >> 8) & 15;  // this token's own width (<= b, the union)
-                        if (bt == 0) continue;         // warp-uniform
-                        if (bt == b) {
-                            accumulate_row(V, (uint16_t)(e >> 16), acc[t]);
-                        } else {
-                            const uint32_t mask = 0x01010101u * ((0xFF00u >> bt) & 0xFFu);
-                            uint32_t Vm[8];
+                for (int t = 0; t < T; ++t) {
+                    const uint32_t e = (t == 0) ? m : s_tok[(t - 1) * GQ_G + i];
+                    const int bt = (e >> 8) & 15;  // this token's own width (<= b, the union)
+                    if (bt == 0) continue;         // warp-uniform
+                    if (bt == b) {
+                        accumulate_row(V, (uint16_t)(e >> 16), acc[t]);
+                    } else {
+                        const uint32_t mask = 0x01010101u * ((0xFF00u >> bt) & 0xFFu);
+                        uint32_t Vm[8];
 #pragma unroll
-                            for (int j = 0; j < 8; ++j) Vm[j] = V[j] & mask;
-                            accumulate_row(Vm, (uint16_t)(e >> 16), acc[t]);
-                        }
+                        for (int j = 0; j < 8; ++j) Vm[j] = V[j] & mask;
+                        accumulate_row(Vm, (uint16_t)(e >> 16), acc[t]);
                     }
                 }
+            }
+        };
+
+        // rows [i0, i1) of the item, all of width B (B = 0: any width, read from the schedule), two per iteration:
+        // one wait + warp barrier, two copies issued into the two slots freed by the previous iteration, then the
+        // two rows' expansion and FMAs are independent instruction streams the scheduler can interleave.
+        auto run = [&](auto b_tag, auto hi_tag, int i0, int i1) {
+            constexpr int PAIR = 1;  // 2 (two independent rows per iteration) was measured: no gain, the loop is not ILP-bound
+            int i = i0;
+            for (; i + PAIR <= i1; i += PAIR) {
+                cp_async_wait<RING - 2 - PAIR>();
+                __syncwarp();
+#pragma unroll
+                for (int u = 0; u < PAIR; ++u) issue_next(hi_tag);
+#pragma unroll
+                for (int u = 0; u < PAIR; ++u) consume(b_tag, i + u);
+            }
+            for (; i < i1; ++i) {  // odd tail of a pair run (next_v may run one ahead of a paired schedule: harmless)
+                cp_async_wait<RING - 2 - PAIR>();
+                __syncwarp();
+                issue_next(hi_tag);
+                consume(b_tag, i);
             }
         };
         {
@@ -311,12 +327,10 @@ vmm_main_kernel(int K, int N, int Q, uint32_t rq, int ipw, int Sx, const uint32_
             run(integral_constant<int, 2>{}, LoT{}, r3, r2);
             run(integral_constant<int, 0>{}, LoT{}, r2, n_rows);
         }
-        if (n_rows > 0 && n_rows - first_i < 4) {  // chunks that found no free iteration (short items, small rings)
+        if (n_rows > 0 && next_v < n_rows + 4) {  // scale/zero chunks that found no iteration (short items)
             __syncwarp();
-            for (int c = n_rows - first_i; c < 4; ++c)
-                issue_sz(c, (uint32_t)((first_i + c - 1) & (RING - 1)) * SLOT_BYTES);
+            while (next_v < n_rows + 4) issue_next(LoT{});
         }
-        cp_async_commit();
         cp_async_wait<0>();
 
         // ---- item end: s and z once per (item, column), into the warp's accumulator
@@ -325,7 +339,7 @@ vmm_main_kernel(int K, int N, int Q, uint32_t rq, int ipw, int Sx, const uint32_
             for (int L = 0; L < 4; ++L) {
                 float sf[8], zf[8];
                 if (n_rows > 0) {
-                    const uint8_t* sz = ring + (uint32_t)((first_i + L - 1) & (RING - 1)) * SLOT_BYTES + lane * 16;
+                    const uint8_t* sz = ring + (uint32_t)((n_rows + L) & (RING - 1)) * SLOT_BYTES + lane * 16;
                     const uint4 sv = *reinterpret_cast<const uint4*>(sz);
                     const uint4 zv = *reinterpret_cast<const uint4*>(sz + 512);
                     const uint32_t su[4] = {sv.x, sv.y, sv.z, sv.w}, zu[4] = {zv.x, zv.y, zv.z, zv.w};
