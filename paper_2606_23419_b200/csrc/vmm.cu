@@ -1,23 +1,25 @@
-// vmm.cu — grinqh_vmm: split-K vector-matrix multiply over the bit-planar store (v1).
+// vmm.cu — grinqh_vmm: split-K vector-matrix multiply over the bit-planar store.
 // PAPER.md:85 (reconstruction), :51 (only the needed planes are fetched), :440-444 (prior-art kernel).
 //
 // Work item = (column tile of 1024 columns, group g of 128 rows, sub-chunk q of Q): the positions
-// q, q+Q, q+2Q, ... of the group's (width desc, index asc) list `grows`, so every item of a group
-// sees the same width mix.  A WARP owns `ipw` consecutive items of one column tile and is fully
-// independent of the other warps until the CTA epilogue (no __syncthreads in the row loop):
+// q, q+Q, q+2Q, ... of the group's (width desc, index asc) list, so every item of a group sees the same
+// width mix.  A WARP owns `ipw` consecutive items of one column tile and is fully independent of the other
+// warps until the CTA epilogue (no __syncthreads in the row loop):
 //
-//   meta     lane l turns list positions 4l..4l+3 into s_meta[p] = row | width << 8 | x_fp16 << 16 and the
-//            warp reduces the item's scalars  X = sum_{b_k>0} x_k,  Phi = sum x_k phi_{b_k}  (phi_b = 2^(7-b)).
+//   prologue lanes stage the item's schedule entries (gsched: row | widths | x) and row byte offsets in shared
+//            memory; the warp reduces the item's scalars X = sum_{b_k>0} x_k, Phi = sum x_k phi_{b_k}.
 //   stream   a warp-private ring of RING 1-KB slots in shared memory, filled by cp.async (LDGSTS.128):
 //            one instruction fetches 4 planes x 128 B of a row (lanes 8j..8j+7 copy plane j), so a 4-bit
-//            row costs one and an 8-bit row two; RING-1 rows are in flight while a row is consumed.
-//   expand   lane l reads its plane words (columns 32l..32l+31 of the tile) from the slot, rebuilds the 32
-//            truncated codes in byte lanes (gather.cuh, SIMD 8x8 bit transpose) and does 32 mixed-precision
-//            FMAs  acc[c] += half(code_c) * half(x_k)   (exact product, fp32 accumulate).
+//            row costs one and an 8-bit row two; RING-2 rows are in flight while a row is consumed; the
+//            group's scales and zeros follow the rows through the same ring.
+//   expand   rows are walked in width-class runs (compile-time b = 8 / 4 / 2, generic otherwise); lane l reads
+//            its plane words (columns 32l..32l+31 of the tile), rebuilds the 32 truncated codes in byte lanes
+//            (gather.cuh, SIMD 8x8 bit transpose) and does 32 mixed-precision FMAs
+//            acc[c] += half(code_c) * half(x_k)   (exact product, fp32 accumulate).
 //   item end y_n += s_gn * (A_n + Phi) + z_gn * X  — s and z are applied once per (item, column) and
 //            summed into the warp's shared-memory accumulator.
 // CTA epilogue: the 8 warps' accumulators are added in fixed order and written as one split-K partial
-// part[sx][t][n]; vmm_reduce sums the Sx partials in fixed order.  Everything is deterministic.
+// part[sx][t][n]; the last CTA of the tile (ticket) sums the Sx partials in fixed order.  Deterministic.
 #include "common.cuh"
 #include <type_traits>
 
