@@ -87,7 +87,7 @@ assign_kernel(const uint16_t* __restrict__ x, AssignParams p, uint8_t* __restric
     __shared__ uint16_t tab[MAXG][10];                              // replicated: per-width counts of every group
     __shared__ uint16_t ltab[MAXG][8];                              // local groups: equal-key counts per cut
     __shared__ int s_rowL[NLEVEL][8 * NDIG];                        // this CTA's row sums, one array per level
-    __shared__ int s_pre[8], s_need[8], s_h[8], s_lead[8], s_slot[8], s_tiebase[8], s_tot[10];
+    __shared__ int s_pre[2][8], s_need[8], s_h[8], s_tiebase[8], s_tot[10];  // s_pre: double-buffered by level parity
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int K = p.K, groups = K / GQ_G, nd = p.nd;
@@ -95,8 +95,11 @@ assign_kernel(const uint16_t* __restrict__ x, AssignParams p, uint8_t* __restric
     const int nloc = max(0, min(gpc, groups - gl0));
     const uint32_t lt_mask = (1u << lane) - 1u;
 
-    auto zero_cnt = [&]() {  // only the rows a level can touch
-        uint4* z = reinterpret_cast<uint4*>(cnt);
+    // cnt is used as two regions of 4 slots (64 KB each) alternating between levels, so the region of level l+1 is
+    // cleared while level l runs; with more than 4 distinct cuts a level needs the whole buffer and clears it first.
+    const bool two_regions = nd <= 4;
+    auto zero_region = [&](int level) {
+        uint4* z = reinterpret_cast<uint4*>(cnt + (two_regions ? (level & 1) * (CNT_BYTES / 2) : 0));
         for (int i = tid; i < nd * NDIG * AT / 16; i += AT) z[i] = make_uint4(0, 0, 0, 0);
     };
 
@@ -107,50 +110,60 @@ assign_kernel(const uint16_t* __restrict__ x, AssignParams p, uint8_t* __restric
         // ---- load the token's local groups (raw patterns; the key is pattern & 0x7FFF)
         for (int i = tid; i < nloc * (GQ_G / 4); i += AT)
             reinterpret_cast<uint2*>(xs)[i] = reinterpret_cast<const uint2*>(x + (size_t)t * K + gl0 * GQ_G)[i];
-        zero_cnt();
+        zero_region(0);
         if (tid < 8) {
-            s_pre[tid] = 0;
+            s_pre[0][tid] = (tid < nd) ? 0 : -1 - tid;  // level 0: one empty prefix shared by every cut
             s_need[tid] = (tid < nd) ? p.Cd[tid] : 0;
             s_h[tid] = 0;
-            s_lead[tid] = (tid == 0);  // level 0: one empty prefix, one slot
-            s_slot[tid] = 0;
             s_tiebase[tid] = 0;
         }
         __syncthreads();
 
-        // ---- radix select, 5 + 5 + 5 bits: every distinct cut keeps (prefix, rank still needed inside it)
+        // ---- radix select, 5 + 5 + 5 bits: every distinct cut keeps (prefix, rank still needed inside it);
+        //      cuts with the same prefix share the histogram slot of the lowest such cut
 #pragma unroll 1
         for (int level = 0; level < NLEVEL; ++level) {
             const int sh = 10 - 5 * level;
+            const int* pre = s_pre[level & 1];
+            uint8_t* reg = cnt + (two_regions ? (level & 1) * (CNT_BYTES / 2) : 0);
             // pass: count the digit of every local key whose prefix is live, in this thread's own byte columns
             for (int i = tid; i < nloc * GQ_G; i += AT) {
                 const uint32_t m = xs[i] & 0x7FFFu;
                 const int pe = (int)(m >> (sh + 5));
                 int s = -1;
-                for (int d = 0; d < nd; ++d)
-                    if (s_lead[d] && s_pre[d] == pe) s = d;
+                for (int d = nd - 1; d >= 0; --d)
+                    if (pre[d] == pe) s = d;
                 if (s >= 0) {
-                    uint8_t* c = cnt + ((s * NDIG + (int)((m >> sh) & 31u)) * AT + tid);
+                    uint8_t* c = reg + ((s * NDIG + (int)((m >> sh) & 31u)) * AT + tid);
                     *c = (uint8_t)(*c + 1);
                 }
             }
+            if (two_regions && level + 1 < NLEVEL) zero_region(level + 1);
             __syncthreads();
-            // reduce: a warp sums one row (AT bytes) of a live slot
-            for (int r = warp; r < nd * NDIG; r += AWARPS) {
-                if (!s_lead[r / NDIG]) continue;
-                const uint4 a = reinterpret_cast<const uint4*>(cnt + r * AT)[lane];
-                uint32_t s = 0;
-                s = __dp4a(a.x, 0x01010101u, s); s = __dp4a(a.y, 0x01010101u, s);
-                s = __dp4a(a.z, 0x01010101u, s); s = __dp4a(a.w, 0x01010101u, s);
-                s = __reduce_add_sync(0xffffffffu, s);
-                if (lane == 0) s_rowL[level][r] = (int)s;
+            // reduce: a warp sums rows (AT bytes each) four at a time
+            for (int r0 = warp * 4; r0 < nd * NDIG; r0 += AWARPS * 4) {
+                uint4 a[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) a[u] = reinterpret_cast<const uint4*>(reg + (r0 + u) * AT)[lane];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    uint32_t s = 0;
+                    s = __dp4a(a[u].x, 0x01010101u, s); s = __dp4a(a[u].y, 0x01010101u, s);
+                    s = __dp4a(a[u].z, 0x01010101u, s); s = __dp4a(a[u].w, 0x01010101u, s);
+                    s = __reduce_add_sync(0xffffffffu, s);
+                    if (lane == 0) s_rowL[level][r0 + u] = (int)s;
+                }
             }
             cluster.sync();
             // locate: warp d reads the 8 CTAs' sums of its slot's 32 digits (DSMEM) and scans them from the top;
             // every CTA takes the same decision on its own copy
             if (warp < nd) {
                 const int d = warp, digit = NDIG - 1 - lane;
-                const int idx = level * (8 * NDIG) + s_slot[d] * NDIG + digit;
+                const int pr = pre[d];
+                int sl = d;
+                for (int e = d - 1; e >= 0; --e)
+                    if (pre[e] == pr) sl = e;
+                const int idx = level * (8 * NDIG) + sl * NDIG + digit;
                 int h = 0, mine_below = 0;
                 for (int r = 0; r < NC; ++r) {
                     const int v = cluster.map_shared_rank(&s_rowL[0][0], r)[idx];
@@ -158,33 +171,24 @@ assign_kernel(const uint16_t* __restrict__ x, AssignParams p, uint8_t* __restric
                     if (r < rank) mine_below += v;
                 }
                 const int incl = warp_incl_scan(h, lane);
-                const int above = incl - h, need = s_need[d], pr = s_pre[d];
+                const int above = incl - h, need = s_need[d];
                 __syncwarp();
                 if (above < need && need <= above + h) {
-                    s_pre[d] = (pr << 5) | digit;
+                    s_pre[(level + 1) & 1][d] = (pr << 5) | digit;
                     s_need[d] = need - above;
                     s_h[d] = h;
                     s_tiebase[d] = mine_below;  // after the last level: keys equal to the cut in lower-ranked CTAs
                 }
             }
+            if (!two_regions && level + 1 < NLEVEL) zero_region(level + 1);
+            if (tid >= 8 * 32 && tid < 8 * 32 + 8 && tid - 8 * 32 >= nd) s_pre[(level + 1) & 1][tid - 8 * 32] = -1 - (tid - 8 * 32);
             __syncthreads();
-            if (level + 1 < NLEVEL) {
-                if (tid < 8) {  // slots of the next level: cuts with the same prefix share one
-                    int sl = tid;
-                    for (int e = tid - 1; e >= 0; --e)
-                        if (s_pre[e] == s_pre[tid]) sl = e;
-                    s_slot[tid] = sl;
-                    s_lead[tid] = (tid < nd && sl == tid);
-                }
-                zero_cnt();
-                __syncthreads();
-            }
         }
         int thr[8], take[8], mult[8];
         bool split[8], anysplit = false;
 #pragma unroll
         for (int d = 0; d < 8; ++d) {
-            thr[d] = (d < nd) ? s_pre[d] : 0x8000;
+            thr[d] = (d < nd) ? s_pre[NLEVEL & 1][d] : 0x8000;
             take[d] = (d < nd) ? s_need[d] : 0;
             mult[d] = (d < nd) ? p.mult[d] : 0;
             split[d] = (d < nd) && take[d] < s_h[d];
