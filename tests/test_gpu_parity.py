@@ -252,3 +252,17 @@ def test_fused_second_pass_matches_two_launches_and_workspace_is_reusable(gq):
             y2 = torch.empty((T, N), dtype=torch.float32, device="cuda")
             gq.grinqh_vmm_reduce(T, K, N, y2, ws)
             assert np.array_equal(y1, y2.cpu().numpy())
+
+
+@pytest.mark.parametrize("T,K,N,mix,seed", [(1, 128, 32, "4", 1), (4, 1024, 96, "2", 3), (3, 640, 1184, "5", 5),
+                                            (1, 4096, 1024, "0", 6), (2, 256, 4096 + 32, "8", 7)])
+def test_vmm_edge_shapes(gq, T, K, N, mix, seed):
+    """smallest legal shape, ragged tiles (N % 128 != 0 -> 4-byte copy path), all-zero and all-8-bit mixes, T up to 4"""
+    W = synth.make_weights(K, N, 0.02, seed)
+    x = synth.make_x(T, K, seed, "student_t")
+    y, y_ref = _run_vmm(gq, W, x, synth.MIXES[mix])
+    if mix == "0":
+        assert not y.any() and not y_ref.any()
+    else:
+        for t in range(T):
+            assert rel_l2(y[t], y_ref[t]) <= TOL
