@@ -119,6 +119,24 @@ int grinqh_assign(const void* x_f16, int T, int K, const uint32_t counts[9],
                   void* workspace, size_t workspace_bytes, void* stream);
 
 /*
+ * grinqh_assign_thresholds — the paper's own run-time form (b_i = b_k if |x_i| in
+ * [theta_k, theta_{k+1}); "negligible latency", :73).  No ranking: b = max{w : m >= theta[w]} on the 15 magnitude
+ * bits m of the fp16 pattern; the effective bits then float around the calibration target instead of hitting it
+ * exactly.  Everything after the widths (union, rows, cnt_ge, grows, gcnt_ge, gsched) is as in grinqh_assign.
+ *   theta   HOST [9] fp16 magnitude patterns, theta[w] (w = 1..8) = smallest magnitude that still gets >= w bits,
+ *           non-decreasing in w, 0x8000 = width w unreachable; theta[0] ignored.  GRINQH_ERR_MIX if not monotone.
+ *
+ * grinqh_calibrate_thresholds — offline HOST helper (Eq. 2): for each of the S calibration
+ * vectors the magnitude that separates the levels under the rank partition `counts` (the C_w-th largest |x|),
+ * averaged in fp64, rounded to fp32 then fp16 (round-to-nearest-even); C_w == 0 -> 0x8000.
+ *   x_host_f16  HOST [S, K] fp16      counts HOST [9], sum = K      theta HOST [9], written
+ */
+int grinqh_assign_thresholds(const void* x_f16, int T, int K, const uint16_t theta[9],
+                             uint8_t* bits, uint8_t* bits_union, int32_t* rows, int32_t* cnt_ge,
+                             uint8_t* grows, uint8_t* gcnt_ge, uint32_t* gsched, void* stream);
+int grinqh_calibrate_thresholds(const void* x_host_f16, int S, int K, const uint32_t counts[9], uint16_t theta[9]);
+
+/*
  * grinqh_vmm — per projection (PAPER.md:85 reconstruction, :51 selective fetch).
  * ONE launch: split-K main kernel (warps walk the per-group schedule and fetch only planes j < bits_union[k] of
  * row k) whose last-finishing CTA per column tile runs the deterministic second pass: it sums the tile's split-K

@@ -112,6 +112,43 @@ def assign(x, counts, G: int = 128):
     return out
 
 
+def assign_thresholds(x, theta, G: int = 128):
+    """Threshold form.  theta: 9 fp16 magnitude patterns (uint16), theta[w] = smallest magnitude
+    that still gets >= w bits (0x8000 = unreachable), theta[0] ignored.  Same outputs as assign()."""
+    xb = _u16(x)
+    if xb.ndim == 1:
+        xb = xb[None, :]
+    T, K = xb.shape
+    theta = np.ascontiguousarray(theta, dtype=np.uint16)
+    assert theta.shape == (9,)
+    out = dict(
+        bits=np.zeros((T, K), dtype=np.uint8),
+        bits_union=np.zeros(K, dtype=np.uint8),
+        rows=np.zeros(K, dtype=np.int32),
+        cnt_ge=np.zeros(10, dtype=np.int32),
+        grows=np.zeros(K, dtype=np.uint8),
+        gcnt_ge=np.zeros((K // G, GCNT_STRIDE), dtype=np.uint8),
+    )
+    rc = lib().orc_assign_thresholds(_p(xb), T, K, G, _p(theta), _p(out["bits"]), _p(out["bits_union"]),
+                                     _p(out["rows"]), _p(out["cnt_ge"]), _p(out["grows"]), _p(out["gcnt_ge"]),
+                                     GCNT_STRIDE)
+    if rc:
+        raise ValueError(f"orc_assign_thresholds failed: {rc}")
+    return out
+
+
+def calibrate_thresholds(xs, counts) -> np.ndarray:
+    """xs [S, K] fp16 calibration vectors -> theta [9] uint16 (Eq. 2: mean split magnitudes)."""
+    xb = _u16(xs)
+    S, K = xb.shape
+    counts = np.ascontiguousarray(counts, dtype=np.uint32)
+    theta = np.zeros(9, dtype=np.uint16)
+    rc = lib().orc_calibrate_thresholds(_p(xb), S, K, _p(counts), _p(theta))
+    if rc:
+        raise ValueError(f"orc_calibrate_thresholds failed: {rc}")
+    return theta
+
+
 def _vmm_args(x, planes, scales, zeros, bits):
     xb = _u16(x)
     if xb.ndim == 1:

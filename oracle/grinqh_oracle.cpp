@@ -214,32 +214,10 @@ int orc_rank_bruteforce(const uint16_t* x, int K, int32_t* rank) {
     return 0;
 }
 
-// c.2 — rank / top-p assignment (PAPER.md:61-65 with the per-vector top-p partition of :271).
-int orc_assign(const uint16_t* x, int T, int K, int G, const uint32_t* counts, uint8_t* bits, uint8_t* bits_union,
-               int32_t* rows, int32_t* cnt_ge, uint8_t* grows, uint8_t* gcnt_ge, int gcnt_stride) {
-    if (K % G || G > 256) return -2;
-    unsigned long long total = 0;
-    for (int w = 0; w < 9; ++w) total += counts[w];
-    if (total != (unsigned long long)K) return -4;
-    long long C[10];
-    C[9] = 0;
-    for (int w = 8; w >= 0; --w) C[w] = C[w + 1] + counts[w];
+// union over tokens and the compacted lists from per-token widths (shared by the rank and threshold forms)
+static void lists_from_bits(const uint8_t* bits, int T, int K, int G, uint8_t* bits_union, int32_t* rows,
+                            int32_t* cnt_ge, uint8_t* grows, uint8_t* gcnt_ge, int gcnt_stride) {
     std::vector<int32_t> order(K);
-    for (int t = 0; t < T; ++t) {
-        const uint16_t* xt = x + (size_t)t * K;
-        std::iota(order.begin(), order.end(), 0);
-        std::stable_sort(order.begin(), order.end(),
-                         [&](int32_t a, int32_t b) { return (xt[a] & 0x7FFF) > (xt[b] & 0x7FFF); });
-        for (int r = 0; r < K; ++r) {
-            int b = 0;
-            for (int w = 8; w >= 1; --w)
-                if (r < C[w]) {
-                    b = w;
-                    break;
-                }
-            bits[(size_t)t * K + order[r]] = (uint8_t)b;
-        }
-    }
     for (int k = 0; k < K; ++k) {
         uint8_t m = 0;
         for (int t = 0; t < T; ++t) m = std::max(m, bits[(size_t)t * K + k]);
@@ -268,6 +246,81 @@ int orc_assign(const uint16_t* x, int T, int K, int G, const uint32_t* counts, u
             gcnt_ge[(size_t)g * gcnt_stride + w] = (uint8_t)c;
         }
     }
+}
+
+
+// c.2 — rank / top-p assignment (PAPER.md:61-65 with the per-vector top-p partition of :271).
+int orc_assign(const uint16_t* x, int T, int K, int G, const uint32_t* counts, uint8_t* bits, uint8_t* bits_union,
+               int32_t* rows, int32_t* cnt_ge, uint8_t* grows, uint8_t* gcnt_ge, int gcnt_stride) {
+    if (K % G || G > 256) return -2;
+    unsigned long long total = 0;
+    for (int w = 0; w < 9; ++w) total += counts[w];
+    if (total != (unsigned long long)K) return -4;
+    long long C[10];
+    C[9] = 0;
+    for (int w = 8; w >= 0; --w) C[w] = C[w + 1] + counts[w];
+    std::vector<int32_t> order(K);
+    for (int t = 0; t < T; ++t) {
+        const uint16_t* xt = x + (size_t)t * K;
+        std::iota(order.begin(), order.end(), 0);
+        std::stable_sort(order.begin(), order.end(),
+                         [&](int32_t a, int32_t b) { return (xt[a] & 0x7FFF) > (xt[b] & 0x7FFF); });
+        for (int r = 0; r < K; ++r) {
+            int b = 0;
+            for (int w = 8; w >= 1; --w)
+                if (r < C[w]) {
+                    b = w;
+                    break;
+                }
+            bits[(size_t)t * K + order[r]] = (uint8_t)b;
+        }
+    }
+    lists_from_bits(bits, T, K, G, bits_union, rows, cnt_ge, grows, gcnt_ge, gcnt_stride);
+    return 0;
+}
+
+// f1 — threshold assignment, the paper's run-time form (b_i = b_k if |x_i| in [theta_k, theta_{k+1})).
+// theta[w], w = 1..8: the smallest fp16 magnitude pattern that still gets at least w bits, non-decreasing in w;
+// 0x8000 (above every magnitude) = width w is unreachable.  theta[0] is ignored.  b = max{w : m >= theta[w]}.
+int orc_assign_thresholds(const uint16_t* x, int T, int K, int G, const uint16_t* theta, uint8_t* bits,
+                          uint8_t* bits_union, int32_t* rows, int32_t* cnt_ge, uint8_t* grows, uint8_t* gcnt_ge,
+                          int gcnt_stride) {
+    if (K % G || G > 256) return -2;
+    for (int w = 2; w <= 8; ++w)
+        if (theta[w] < theta[w - 1] || theta[w] > 0x8000) return -4;
+    for (int t = 0; t < T; ++t)
+        for (int k = 0; k < K; ++k) {
+            const int m = x[(size_t)t * K + k] & 0x7FFF;
+            int b = 0;
+            for (int w = 1; w <= 8; ++w)
+                if (m >= (int)theta[w]) b = w;
+            bits[(size_t)t * K + k] = (uint8_t)b;
+        }
+    lists_from_bits(bits, T, K, G, bits_union, rows, cnt_ge, grows, gcnt_ge, gcnt_stride);
+    return 0;
+}
+
+// Calibration of the thresholds (Eq. 2): for every calibration vector the magnitude that
+// separates the levels under the rank partition (the C_w-th largest |x|, i.e. the smallest one that still gets
+// >= w bits), averaged over the S vectors in fp64, rounded to fp32 and then to fp16 (both round-to-nearest-even).
+// C_w == 0 -> 0x8000 (unreachable).
+int orc_calibrate_thresholds(const uint16_t* xs, int S, int K, const uint32_t* counts, uint16_t* theta) {
+    unsigned long long total = 0;
+    for (int w = 0; w < 9; ++w) total += counts[w];
+    if (total != (unsigned long long)K || S < 1) return -4;
+    long long C[10];
+    C[9] = 0;
+    for (int w = 8; w >= 0; --w) C[w] = C[w + 1] + counts[w];
+    std::vector<int> mags(K);
+    double sum[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};
+    for (int s = 0; s < S; ++s) {
+        for (int k = 0; k < K; ++k) mags[k] = xs[(size_t)s * K + k] & 0x7FFF;
+        std::sort(mags.begin(), mags.end(), [](int a, int b) { return a > b; });
+        for (int w = 1; w <= 8; ++w)
+            if (C[w] > 0) sum[w] += (double)half_to_float((uint16_t)mags[C[w] - 1]);
+    }
+    theta[0] = 0;
+    for (int w = 1; w <= 8; ++w) theta[w] = (C[w] > 0) ? float_to_half((float)(sum[w] / S)) : (uint16_t)0x8000;
     return 0;
 }
 

@@ -37,6 +37,10 @@ _lib.grinqh_assign_workspace_bytes.restype = _sz
 _lib.grinqh_assign_workspace_bytes.argtypes = [_i, _i]
 _lib.grinqh_assign.restype = _i
 _lib.grinqh_assign.argtypes = [_vp, _i, _i, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _sz, _vp]
+_lib.grinqh_assign_thresholds.restype = _i
+_lib.grinqh_assign_thresholds.argtypes = [_vp, _i, _i, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp]
+_lib.grinqh_calibrate_thresholds.restype = _i
+_lib.grinqh_calibrate_thresholds.argtypes = [_vp, _i, _i, _vp, _vp]
 _lib.grinqh_vmm_workspace_bytes.restype = _sz
 _lib.grinqh_vmm_workspace_bytes.argtypes = [_i, _i, _i]
 _lib.grinqh_vmm_workspace_init.restype = _i
@@ -53,7 +57,8 @@ _lib.grinqh_decode_host.argtypes = [_vp, _i, _i, _i, _i, _vp, _vp, _vp, _vp, _vp
                                     _vp, _vp, _sz, _vp, _vp, _sz, _vp, _i, _vp]
 
 EXPORTS = ("grinqh_status_string", "grinqh_version", "grinqh_mix_to_counts", "grinqh_pack",
-           "grinqh_assign_workspace_bytes", "grinqh_assign", "grinqh_vmm_workspace_bytes",
+           "grinqh_assign_workspace_bytes", "grinqh_assign", "grinqh_assign_thresholds",
+           "grinqh_calibrate_thresholds", "grinqh_vmm_workspace_bytes",
            "grinqh_vmm_workspace_init", "grinqh_vmm",
            "grinqh_vmm_main", "grinqh_vmm_reduce", "grinqh_decode_host")
 
@@ -139,6 +144,29 @@ def grinqh_assign(x: torch.Tensor, counts, out: Assignment | None = None, stream
                               _stream(stream)),
            "grinqh_assign")
     return out
+
+
+def grinqh_assign_thresholds(x: torch.Tensor, theta, out: Assignment | None = None, stream=None) -> Assignment:
+    """Threshold form of the assignment; theta: 9 uint16 fp16-magnitude patterns (theta[0] unused)."""
+    T, K = x.shape
+    out = out or Assignment(T, K, x.device)
+    th = (C.c_uint16 * 9)(*[int(v) for v in theta])
+    _check(_lib.grinqh_assign_thresholds(_dev(x, torch.float16, "x"), T, K, th, out.bits.data_ptr(),
+                                         out.bits_union.data_ptr(), out.rows.data_ptr(), out.cnt_ge.data_ptr(),
+                                         out.grows.data_ptr(), out.gcnt_ge.data_ptr(), out.gsched.data_ptr(),
+                                         _stream(stream)), "grinqh_assign_thresholds")
+    return out
+
+
+def grinqh_calibrate_thresholds(xs_host: torch.Tensor, counts) -> list[int]:
+    """HOST xs [S, K] fp16 calibration vectors -> theta [9] uint16 patterns."""
+    if xs_host.is_cuda or xs_host.dtype != torch.float16 or not xs_host.is_contiguous():
+        raise GrinqhError("grinqh_calibrate_thresholds takes a contiguous HOST fp16 tensor [S, K]")
+    S, K = xs_host.shape
+    th = (C.c_uint16 * 9)()
+    _check(_lib.grinqh_calibrate_thresholds(xs_host.data_ptr(), S, K, _counts(counts), th),
+           "grinqh_calibrate_thresholds")
+    return [int(v) for v in th]
 
 
 def grinqh_vmm_workspace_bytes(T: int, K: int, N: int) -> int:

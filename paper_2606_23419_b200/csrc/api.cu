@@ -1,6 +1,10 @@
 // api.cu — host-side entry points of the C ABI that launch no kernel of their own.
 #include <math.h>
 
+#include <algorithm>
+#include <functional>
+#include <vector>
+
 #include "common.cuh"
 
 extern "C" const char* grinqh_status_string(int status) {
@@ -40,6 +44,44 @@ extern "C" int grinqh_mix_to_counts(int K, const double frac[9], uint32_t counts
     }
     C[0] = K;
     for (int w = 0; w < 9; ++w) counts[w] = (uint32_t)(C[w] - C[w + 1]);
+    return GRINQH_OK;
+}
+
+// PAPER.md:69-73, :271-273 (Eq. 2): thresholds = per-vector level-separating magnitudes under the rank partition,
+// averaged over the calibration vectors.  Offline host helper (like grinqh_mix_to_counts): fp64 mean of the C_w-th
+// largest |x| of every vector, rounded to fp32 then fp16 (RN-even); C_w == 0 -> 0x8000 (width w unreachable).
+extern "C" int grinqh_calibrate_thresholds(const void* x_host_f16, int S, int K, const uint32_t counts[9],
+                                           uint16_t theta[9]) {
+    if (!x_host_f16 || !counts || !theta) return GRINQH_ERR_NULL;
+    if (S < 1 || K <= 0) return GRINQH_ERR_SHAPE;
+    unsigned long long total = 0;
+    for (int w = 0; w < 9; ++w) total += counts[w];
+    if (total != (unsigned long long)K) return GRINQH_ERR_MIX;
+    long long C[10];
+    C[9] = 0;
+    for (int w = 8; w >= 0; --w) C[w] = C[w + 1] + counts[w];
+    const uint16_t* x = (const uint16_t*)x_host_f16;
+    std::vector<uint16_t> m((size_t)K);
+    double sum[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};
+    for (int s = 0; s < S; ++s) {
+        for (int k = 0; k < K; ++k) m[k] = x[(size_t)s * K + k] & 0x7FFFu;
+        for (int w = 1; w <= 8; ++w) {
+            if (C[w] == 0) continue;
+            std::nth_element(m.begin(), m.begin() + (C[w] - 1), m.end(), std::greater<uint16_t>());
+            __half_raw r;
+            r.x = m[C[w] - 1];
+            sum[w] += (double)__half2float(__half(r));
+        }
+    }
+    theta[0] = 0;
+    for (int w = 1; w <= 8; ++w) {
+        if (C[w] == 0) {
+            theta[w] = 0x8000;
+        } else {
+            const __half_raw r = __float2half_rn((float)(sum[w] / S));
+            theta[w] = r.x;
+        }
+    }
     return GRINQH_OK;
 }
 

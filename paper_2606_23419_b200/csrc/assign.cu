@@ -36,6 +36,8 @@ struct AssignParams {
     int Cd[8];    // their ranks: the Cd[d] largest keys are "above" cut d
     int mult[8];  // how many widths w share the cut: b = sum_d mult[d] * [above cut d]
     int C[10];    // C[w] = rows with width >= w (for cnt_ge bookkeeping only)
+    int use_thr;  // threshold form (grinqh_assign_thresholds): no selection, the cut keys are given
+    int thr[8];   // use_thr: key of distinct cut d ("above" = magnitude pattern >= thr[d])
 };
 
 __device__ __forceinline__ int warp_incl_scan(int v, int lane) {
@@ -119,10 +121,18 @@ assign_kernel(const uint16_t* __restrict__ x, AssignParams p, uint8_t* __restric
         }
         __syncthreads();
 
+        if (p.use_thr) {  // the paper's run-time form: static thresholds, nothing to select
+            if (tid < 8) {
+                s_pre[NLEVEL & 1][tid] = (tid < nd) ? p.thr[tid] : 0x8000;
+                s_need[tid] = 0;
+                s_h[tid] = 0;  // take == h == 0: no cut splits a tie run, every key >= thr is above the cut
+            }
+            __syncthreads();
+        }
         // ---- radix select, 5 + 5 + 5 bits: every distinct cut keeps (prefix, rank still needed inside it);
         //      cuts with the same prefix share the histogram slot of the lowest such cut
 #pragma unroll 1
-        for (int level = 0; level < NLEVEL; ++level) {
+        for (int level = p.use_thr ? NLEVEL : 0; level < NLEVEL; ++level) {
             const int sh = 10 - 5 * level;
             const int* pre = s_pre[level & 1];
             uint8_t* reg = cnt + (two_regions ? (level & 1) * (CNT_BYTES / 2) : 0);
@@ -399,17 +409,59 @@ extern "C" size_t grinqh_assign_workspace_bytes(int T, int K) {
     return 0;  // everything lives in shared memory; the argument is kept for ABI stability
 }
 
-extern "C" int grinqh_assign(const void* x_f16, int T, int K, const uint32_t counts[9], uint8_t* bits,
-                             uint8_t* bits_union, int32_t* rows, int32_t* cnt_ge, uint8_t* grows, uint8_t* gcnt_ge,
-                             uint32_t* gsched, void* workspace, size_t workspace_bytes, void* stream) {
-    (void)workspace;
-    (void)workspace_bytes;
-    if (!x_f16 || !counts || !bits || !bits_union || !rows || !cnt_ge || !grows || !gcnt_ge || !gsched)
+namespace gq {
+static int check_assign_args(const void* x_f16, int T, int K, const void* spec, uint8_t* bits, uint8_t* bits_union,
+                             int32_t* rows, int32_t* cnt_ge, uint8_t* grows, uint8_t* gcnt_ge, uint32_t* gsched) {
+    if (!x_f16 || !spec || !bits || !bits_union || !rows || !cnt_ge || !grows || !gcnt_ge || !gsched)
         return GRINQH_ERR_NULL;
     if (T < 1 || T > GRINQH_MAX_T || K <= 0 || K % GQ_G || K > GQ_MAX_K) return GRINQH_ERR_SHAPE;
     if (((uintptr_t)x_f16 | (uintptr_t)bits | (uintptr_t)bits_union | (uintptr_t)rows | (uintptr_t)cnt_ge |
          (uintptr_t)grows | (uintptr_t)gcnt_ge | (uintptr_t)gsched) & 15)
         return GRINQH_ERR_ALIGN;
+    return GRINQH_OK;
+}
+
+static int launch_assign(const AssignParams& p, const void* x_f16, uint8_t* bits, uint8_t* bits_union, int32_t* rows,
+                         int32_t* cnt_ge, uint8_t* grows, uint8_t* gcnt_ge, uint32_t* gsched, void* stream) {
+    // cluster size: measured on B200 (T=1, K=4096): 1 CTA 23.5 us, 2: 16.4, 4: 13.4, 8: 12.3 — the kernel is bound by
+    // per-CTA instruction latency, not by the cluster barriers, so always the portable maximum
+    const int nc = MAXNC;
+    const int gpc = (p.K / GQ_G + nc - 1) / nc;
+    const size_t smem = (size_t)CNT_BYTES + (size_t)gpc * GQ_G * 3;
+    static bool configured = false;
+    if (!configured) {
+        if (cudaFuncSetAttribute(assign_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 CNT_BYTES + 32 * GQ_G * 3) != cudaSuccess)  // at most 32 groups per CTA
+            return GRINQH_ERR_CUDA;
+        configured = true;
+    }
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(nc);
+    cfg.blockDim = dim3(AT);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = (cudaStream_t)stream;
+    cudaLaunchAttribute at[2];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    at[1].id = cudaLaunchAttributeClusterDimension;
+    at[1].val.clusterDim.x = nc;
+    at[1].val.clusterDim.y = 1;
+    at[1].val.clusterDim.z = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = 2;
+    const cudaError_t e = cudaLaunchKernelEx(&cfg, assign_kernel, (const uint16_t*)x_f16, p, bits, bits_union, rows,
+                                             cnt_ge, grows, gcnt_ge, gsched);
+    return e == cudaSuccess ? GRINQH_OK : GRINQH_ERR_CUDA;
+}
+}  // namespace gq
+
+extern "C" int grinqh_assign(const void* x_f16, int T, int K, const uint32_t counts[9], uint8_t* bits,
+                             uint8_t* bits_union, int32_t* rows, int32_t* cnt_ge, uint8_t* grows, uint8_t* gcnt_ge,
+                             uint32_t* gsched, void* workspace, size_t workspace_bytes, void* stream) {
+    (void)workspace;
+    (void)workspace_bytes;
+    int rc = gq::check_assign_args(x_f16, T, K, counts, bits, bits_union, rows, cnt_ge, grows, gcnt_ge, gsched);
+    if (rc != GRINQH_OK) return rc;
     unsigned long long total = 0;
     for (int w = 0; w < 9; ++w) total += counts[w];
     if (total != (unsigned long long)K) return GRINQH_ERR_MIX;
@@ -428,33 +480,29 @@ extern "C" int grinqh_assign(const void* x_f16, int T, int K, const uint32_t cou
         }
         p.mult[d]++;
     }
-    // cluster size: measured on B200 (T=1, K=4096): 1 CTA 23.5 us, 2: 16.4, 4: 13.4, 8: 12.3 — the kernel is bound by
-    // per-CTA instruction latency, not by the cluster barriers, so always the portable maximum
-    const int nc = gq::MAXNC;
-    const int gpc = (K / GQ_G + nc - 1) / nc;
-    const size_t smem = (size_t)gq::CNT_BYTES + (size_t)gpc * GQ_G * 3;
-    static bool configured = false;
-    if (!configured) {
-        if (cudaFuncSetAttribute(gq::assign_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 gq::CNT_BYTES + 32 * GQ_G * 3) != cudaSuccess)  // at most 32 groups per CTA
-            return GRINQH_ERR_CUDA;
-        configured = true;
+    return gq::launch_assign(p, x_f16, bits, bits_union, rows, cnt_ge, grows, gcnt_ge, gsched, stream);
+}
+
+extern "C" int grinqh_assign_thresholds(const void* x_f16, int T, int K, const uint16_t theta[9], uint8_t* bits,
+                                        uint8_t* bits_union, int32_t* rows, int32_t* cnt_ge, uint8_t* grows,
+                                        uint8_t* gcnt_ge, uint32_t* gsched, void* stream) {
+    int rc = gq::check_assign_args(x_f16, T, K, theta, bits, bits_union, rows, cnt_ge, grows, gcnt_ge, gsched);
+    if (rc != GRINQH_OK) return rc;
+    for (int w = 1; w <= 8; ++w)
+        if (theta[w] > 0x8000 || (w > 1 && theta[w] < theta[w - 1])) return GRINQH_ERR_MIX;
+    gq::AssignParams p{};
+    p.T = T;
+    p.K = K;
+    p.use_thr = 1;
+    for (int w = 1; w <= 8; ++w) {  // distinct reachable thresholds
+        if (theta[w] == 0x8000) continue;
+        int d = 0;
+        while (d < p.nd && p.thr[d] != (int)theta[w]) ++d;
+        if (d == p.nd) {
+            p.thr[p.nd] = (int)theta[w];
+            p.mult[p.nd++] = 0;
+        }
+        p.mult[d]++;
     }
-    cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3(nc);
-    cfg.blockDim = dim3(gq::AT);
-    cfg.dynamicSmemBytes = smem;
-    cfg.stream = (cudaStream_t)stream;
-    cudaLaunchAttribute at[2];
-    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    at[0].val.programmaticStreamSerializationAllowed = 1;
-    at[1].id = cudaLaunchAttributeClusterDimension;
-    at[1].val.clusterDim.x = nc;
-    at[1].val.clusterDim.y = 1;
-    at[1].val.clusterDim.z = 1;
-    cfg.attrs = at;
-    cfg.numAttrs = 2;
-    const cudaError_t e = cudaLaunchKernelEx(&cfg, gq::assign_kernel, (const uint16_t*)x_f16, p, bits, bits_union, rows,
-                                             cnt_ge, grows, gcnt_ge, gsched);
-    return e == cudaSuccess ? GRINQH_OK : GRINQH_ERR_CUDA;
+    return gq::launch_assign(p, x_f16, bits, bits_union, rows, cnt_ge, grows, gcnt_ge, gsched, stream);
 }

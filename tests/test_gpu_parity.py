@@ -266,3 +266,42 @@ def test_vmm_edge_shapes(gq, T, K, N, mix, seed):
     else:
         for t in range(T):
             assert rel_l2(y[t], y_ref[t]) <= TOL
+
+
+@pytest.mark.parametrize("T,K,mix,dist,seed", [(1, 4096, "4", "normal", 0), (2, 8192, "3", "student_t", 1),
+                                               (4, 1536, "2", "normal", 2), (1, 28672, "4", "student_t", 3)])
+def test_assign_thresholds_and_calibration_bit_exact(gq, T, K, mix, dist, seed):
+    """calibration on 8 synthetic vectors, threshold assignment of a
+    fresh one; theta, widths, lists and schedule bit-exact against the oracle; the VMM consumes it unchanged."""
+    counts = oracle.mix_to_counts(K, synth.MIXES[mix])
+    xs = np.concatenate([synth.make_x(1, K, 100 + seed * 10 + s, dist) for s in range(8)], axis=0)
+    theta_ref = oracle.calibrate_thresholds(xs, counts)
+    theta = gq.grinqh_calibrate_thresholds(torch.from_numpy(xs), counts)
+    assert list(theta_ref) == theta
+    x = synth.make_x(T, K, 500 + seed, dist)
+    ref = oracle.assign_thresholds(x, theta_ref)
+    a = gq.grinqh_assign_thresholds(_dev(x), theta)
+    torch.cuda.synchronize()
+    _check_assign(ref, a, x)
+    avg = ref["bits"].mean()
+    assert abs(avg - synth.mix_avg_bits(synth.MIXES[mix])) < 0.5      # floats around the target (Fig. 6B)
+    if K <= 8192:
+        N = 1024
+        W = synth.make_weights(K, N, 0.02, seed)
+        planes, s, z = oracle.pack(W)
+        y_ref = oracle.vmm(x, planes, s, z, ref["bits"])
+        y = gq.grinqh_vmm(gq.grinqh_pack(_dev(W)), a).cpu().numpy()
+        for t in range(T):
+            assert rel_l2(y[t], y_ref[t]) <= TOL
+
+
+def test_assign_thresholds_extremes(gq):
+    K = 2048
+    x = synth.make_x(2, K, 5)
+    for theta in ([0] * 9, [0x8000] * 9, [0, 0, 0, 0x3C00, 0x3C00, 0x4400, 0x8000, 0x8000, 0x8000]):
+        ref = oracle.assign_thresholds(x, np.array(theta, np.uint16))
+        a = gq.grinqh_assign_thresholds(_dev(x), theta)
+        torch.cuda.synchronize()
+        _check_assign(ref, a, x)
+    with pytest.raises(gq.GrinqhError):
+        gq.grinqh_assign_thresholds(_dev(x), [0, 5, 4, 5, 5, 5, 5, 5, 5])
