@@ -267,6 +267,16 @@ def run_native(args):
                 seen.add(inp)
             gq.grinqh_vmm(packed_split[l][name], assigns[l][inp], y_dev[l][name], ws)
 
+    # threshold form: thetas calibrated offline on 8 synthetic vectors per input
+    thetas = {n: gq.grinqh_calibrate_thresholds(
+        torch.from_numpy(np.concatenate([synth.make_x(1, K, 7000 + 10 * i + s, "normal") for s in range(8)], axis=0)),
+        counts[K]) for i, (n, K) in enumerate(in_dims.items())}
+
+    def step_thresholds(l):      # the same step with the paper's threshold assignment instead of the rank form
+        for name, K, N, inp in fused:
+            gq.grinqh_assign_thresholds(x_dev[l][inp], thetas[inp], assigns[l][inp])
+            gq.grinqh_vmm(packed[l][name], assigns[l][inp], y_dev[l][name], ws)
+
     def step_main_only(l):       # the dominant kernel alone: the 4 VMM launches (assignments already on the device)
         for name, K, N, inp in fused:
             gq.grinqh_vmm(packed[l][name], assigns[l][inp], y_dev[l][name], ws)
@@ -329,6 +339,17 @@ def run_native(args):
         for i in range(3):
             g_host[i % L].replay()
         ms_host = timed(g_host, args.steps, sync_each=True)
+        step_thresholds(0)
+        stream.synchronize()
+        g_thr = capture(step_thresholds)
+        for i in range(3):
+            g_thr[i % L].replay()
+        ms_thr = timed(g_thr, args.steps)
+        thr_bits = float(np.mean([assigns[0][n].bits.float().mean().item() for n in in_dims]))
+        for l in range(L):       # leave the rank-form assignments in the buffers (byte accounting below)
+            for n, K in in_dims.items():
+                gq.grinqh_assign(x_dev[l][n], counts[K], assigns[l][n])
+        stream.synchronize()
         ms_split = None
         if g_split:
             for i in range(3):
@@ -381,6 +402,10 @@ def run_native(args):
         "pack": {"GBps": pack_bytes / (pack_ms * 1e-3) / 1e9, "ms_per_layer": pack_ms / L},
         "per_vmm": per_vmm,
     }
+    line["threshold_assignment"] = {"value": max_over_ranks([ms_thr], dev)[0] * 1e3 / args.steps, "unit": UNIT,
+                                    "avg_bits_measured": thr_bits,
+                                    "what": "same step with grinqh_assign_thresholds (the paper's run-time form, thetas "
+                                            "calibrated on 8 synthetic vectors) instead of the rank assignment"}
     if ms_split:
         line["per_projection"] = {"value": ms_split * 1e3 / args.steps, "unit": UNIT,
                                   "what": "same step with one VMM launch per projection (4 assigns + 7 VMMs)"}

@@ -20,7 +20,7 @@ extern "C" const char* grinqh_status_string(int status) {
     }
 }
 
-extern "C" int grinqh_version(void) { return 100; /* 0.1.0 */ }
+extern "C" int grinqh_version(void) { return 200; /* 0.2.0: gsched schedule, fused second pass, threshold assignment */ }
 
 // PAPER.md:262-266 (Eq. 1): precision distribution P -> integer row counts; reading #3.
 extern "C" int grinqh_mix_to_counts(int K, const double frac[9], uint32_t counts[9]) {
