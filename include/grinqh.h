@@ -166,6 +166,16 @@ int grinqh_vmm_reduce(int T, int K, int N, float* y,
                       const void* workspace, size_t workspace_bytes, void* stream);
 
 /*
+ * grinqh_vmm_thresholds — the threshold assignment made inside the VMM launch (SURVEY.md 8f4:
+ * assignment fused into its consumer).  Every warp derives the widths, the union and the (width desc, index asc)
+ * list of its 128-row group from x and theta; no assignment kernel runs and no schedule is written.  y is bit-identical
+ * to grinqh_assign_thresholds followed by grinqh_vmm.  Arguments as in those two calls.
+ */
+int grinqh_vmm_thresholds(const void* x_f16, int T, int K, int N, int group, const uint16_t theta[9],
+                          const uint32_t* planes, const void* scales_f16, const void* zeros_f16,
+                          float* y, void* workspace, size_t workspace_bytes, void* stream);
+
+/*
  * Host-buffer decode call (the end-to-end entry): copies x from HOST memory to
  * the device staging buffer x_dev_f16, runs grinqh_assign + grinqh_vmm, and
  * copies y back to HOST memory, all enqueued on `stream` (cudaMemcpyAsync;

@@ -48,6 +48,8 @@ _lib.grinqh_vmm_workspace_init.argtypes = [_vp, _sz, _vp]
 _VMM_COMMON = [_i, _i, _i, _i, _vp, _vp, _vp, _vp, _vp]
 _lib.grinqh_vmm.restype = _i
 _lib.grinqh_vmm.argtypes = _VMM_COMMON + [_vp, _vp, _sz, _vp]
+_lib.grinqh_vmm_thresholds.restype = _i
+_lib.grinqh_vmm_thresholds.argtypes = [_vp, _i, _i, _i, _i, _vp, _vp, _vp, _vp, _vp, _vp, _sz, _vp]
 _lib.grinqh_vmm_main.restype = _i
 _lib.grinqh_vmm_main.argtypes = _VMM_COMMON + [_vp, _sz, _vp]
 _lib.grinqh_vmm_reduce.restype = _i
@@ -59,7 +61,7 @@ _lib.grinqh_decode_host.argtypes = [_vp, _i, _i, _i, _i, _vp, _vp, _vp, _vp, _vp
 EXPORTS = ("grinqh_status_string", "grinqh_version", "grinqh_mix_to_counts", "grinqh_pack",
            "grinqh_assign_workspace_bytes", "grinqh_assign", "grinqh_assign_thresholds",
            "grinqh_calibrate_thresholds", "grinqh_vmm_workspace_bytes",
-           "grinqh_vmm_workspace_init", "grinqh_vmm",
+           "grinqh_vmm_workspace_init", "grinqh_vmm", "grinqh_vmm_thresholds",
            "grinqh_vmm_main", "grinqh_vmm_reduce", "grinqh_decode_host")
 
 
@@ -203,6 +205,20 @@ def grinqh_vmm(w: Packed, a: Assignment, y: torch.Tensor | None = None,
     workspace, nbytes = _ws(T, K, w.N, workspace, dev)
     _check(_lib.grinqh_vmm(*_vmm_common(w, a), _dev(y, torch.float32, "y"), workspace.data_ptr(), nbytes,
                            _stream(stream)), "grinqh_vmm")
+    return y
+
+
+def grinqh_vmm_thresholds(x: torch.Tensor, theta, w: Packed, y: torch.Tensor | None = None,
+                          workspace: torch.Tensor | None = None, stream=None) -> torch.Tensor:
+    """y [T, N] = x . W with the threshold assignment made inside the VMM launch (no assignment kernel)."""
+    T, K = x.shape
+    if y is None:
+        y = torch.empty((T, w.N), dtype=torch.float32, device=x.device)
+    workspace, nbytes = _ws(T, K, w.N, workspace, x.device)
+    th = (C.c_uint16 * 9)(*[int(v) for v in theta])
+    _check(_lib.grinqh_vmm_thresholds(_dev(x, torch.float16, "x"), T, K, w.N, GROUP, th, w.planes.data_ptr(),
+                                      w.scales.data_ptr(), w.zeros.data_ptr(), _dev(y, torch.float32, "y"),
+                                      workspace.data_ptr(), nbytes, _stream(stream)), "grinqh_vmm_thresholds")
     return y
 
 

@@ -287,53 +287,10 @@ assign_kernel(const uint16_t* __restrict__ x, AssignParams p, uint8_t* __restric
                 xv[t] = (p.T == 1) ? *reinterpret_cast<const uint2*>(xs + lo)
                                    : *reinterpret_cast<const uint2*>(x + (size_t)t * K + go);
             }
-        // stable partition of the 128 rows by (width desc, index asc): per-lane counts of the 9 widths packed in
-        // byte fields (widths 0..7 in a u64, width 8 apart; a prefix never exceeds 128), one inclusive warp scan
-        int bu[4], pos[4];
-        unsigned long long cntA = 0;
-        uint32_t cnt8 = 0;
+        int bu[4], pos[4], ge[10];
 #pragma unroll
-        for (int i = 0; i < 4; ++i) {
-            bu[i] = (bu4 >> (8 * i)) & 0xFF;
-            if (bu[i] == 8) ++cnt8;
-            else cntA += 1ull << (8 * bu[i]);
-        }
-        unsigned long long inA = cntA;
-        uint32_t in8 = cnt8;
-#pragma unroll
-        for (int d = 1; d < 32; d <<= 1) {
-            const unsigned long long oA = __shfl_up_sync(0xffffffffu, inA, d);
-            const uint32_t o8 = __shfl_up_sync(0xffffffffu, in8, d);
-            if (lane >= d) {
-                inA += oA;
-                in8 += o8;
-            }
-        }
-        const unsigned long long totA = __shfl_sync(0xffffffffu, inA, 31);
-        const uint32_t tot8 = __shfl_sync(0xffffffffu, in8, 31);
-        unsigned long long exA = inA - cntA;  // rows of each width in lower lanes
-        uint32_t ex8 = in8 - cnt8;
-        // ge[c] = rows of the group with width >= c
-        int ge[10];
-        ge[9] = 0;
-        ge[8] = (int)tot8;
-#pragma unroll
-        for (int c = 7; c >= 0; --c) ge[c] = ge[c + 1] + (int)((totA >> (8 * c)) & 0xFF);
-#pragma unroll
-        for (int i = 0; i < 4; ++i) {
-            const int c = bu[i];
-            int above = 0, lower;  // above = rows of larger width
-#pragma unroll
-            for (int w = 0; w <= 8; ++w)
-                if (w == c) above = ge[w + 1];
-            if (c == 8) {
-                lower = (int)ex8++;
-            } else {
-                lower = (int)((exA >> (8 * c)) & 0xFF);
-                exA += 1ull << (8 * c);
-            }
-            pos[i] = above + lower;
-        }
+        for (int i = 0; i < 4; ++i) bu[i] = (bu4 >> (8 * i)) & 0xFF;
+        partition128(bu, lane, pos, ge);
         int myge = 0, myn = 0;
 #pragma unroll
         for (int c = 0; c <= 8; ++c)

@@ -36,6 +36,54 @@ __device__ __forceinline__ void fhfma_hi(float& acc, uint32_t a, uint16_t x) {
         : "+f"(acc) : "r"(a), "h"(x));
 }
 
+// Stable partition of a 128-row group by (width desc, index asc), one warp, lane l owns rows 4l..4l+3 with widths
+// bu[0..3] (0..8).  Per-lane counts of the 9 widths are packed in byte fields (widths 0..7 in a u64, width 8 apart; a
+// prefix never exceeds 128) and scanned once.  pos[i] = position of row 4l+i in the group's list; ge[c] = rows of
+// width >= c (ge[9] = 0), the same on every lane.
+__device__ __forceinline__ void partition128(const int (&bu)[4], int lane, int (&pos)[4], int (&ge)[10]) {
+    unsigned long long cntA = 0;
+    uint32_t cnt8 = 0;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        if (bu[i] == 8) ++cnt8;
+        else cntA += 1ull << (8 * bu[i]);
+    }
+    unsigned long long inA = cntA;
+    uint32_t in8 = cnt8;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const unsigned long long oA = __shfl_up_sync(0xffffffffu, inA, d);
+        const uint32_t o8 = __shfl_up_sync(0xffffffffu, in8, d);
+        if (lane >= d) {
+            inA += oA;
+            in8 += o8;
+        }
+    }
+    const unsigned long long totA = __shfl_sync(0xffffffffu, inA, 31);
+    const uint32_t tot8 = __shfl_sync(0xffffffffu, in8, 31);
+    unsigned long long exA = inA - cntA;  // rows of each width in lower lanes
+    uint32_t ex8 = in8 - cnt8;
+    ge[9] = 0;
+    ge[8] = (int)tot8;
+#pragma unroll
+    for (int c = 7; c >= 0; --c) ge[c] = ge[c + 1] + (int)((totA >> (8 * c)) & 0xFF);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const int c = bu[i];
+        int above = 0, lower;  // above = rows of larger width
+#pragma unroll
+        for (int w = 0; w <= 8; ++w)
+            if (w == c) above = ge[w + 1];
+        if (c == 8) {
+            lower = (int)ex8++;
+        } else {
+            lower = (int)((exA >> (8 * c)) & 0xFF);
+            exA += 1ull << (8 * c);
+        }
+        pos[i] = above + lower;
+    }
+}
+
 // Programmatic dependent launch (PDL): every per-step kernel is launched with programmatic stream serialization,
 // calls pdl_launch_dependents() at its top (the next kernel of the stream may be scheduled as SMs free up) and
 // pdl_wait() before its first global-memory access (blocks until the previous kernel has completed and flushed).

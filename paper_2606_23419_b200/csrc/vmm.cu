@@ -82,6 +82,12 @@ static inline VmmPlan vmm_plan(int T, int K, int N) {
 // codes are fed to the FMA as fp16 bit patterns 0x00cc = cc * 2^-24 (subnormal halfs, exact)
 constexpr float CODE_SCALE = 16777216.0f;
 
+// threshold assignment done inside the VMM (grinqh_vmm_thresholds): distinct cut keys and how many widths share each
+struct ThrParams {
+    int thr[8];   // magnitude pattern of distinct cut d (0x8000 = unused: no key reaches it)
+    int mult[8];  // widths sharing the cut: b = sum_d mult[d] * [key >= thr[d]]
+};
+
 __device__ __forceinline__ void cp_async16(uint32_t dst, const void* src) {
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
 }
@@ -119,7 +125,8 @@ __global__ void __launch_bounds__(VTHREADS, ctas_per_sm(T))
 vmm_main_kernel(int K, int N, int Q, uint32_t rq, int ipw, int Sx, const uint32_t* __restrict__ planes,
                 const __half* __restrict__ scales, const __half* __restrict__ zeros,
                 const uint32_t* __restrict__ gsched, const uint8_t* __restrict__ gcnt_ge,
-                float* __restrict__ part, int* __restrict__ tickets, float* __restrict__ y) {
+                float* __restrict__ part, int* __restrict__ tickets, float* __restrict__ y,
+                const uint16_t* __restrict__ xraw, ThrParams tp) {
     using C = Cfg<T>;
     constexpr int RING = C::RING;
     constexpr uint32_t RING_MASK = RING * SLOT_BYTES - 1;
@@ -161,17 +168,63 @@ vmm_main_kernel(int K, int N, int Q, uint32_t rq, int ipw, int Sx, const uint32_
         const int g = (int)(((uint32_t)it * rq) >> 16), q = it - g * Q;  // it / Q (rq = ceil(65536 / Q), it < 8192)
         __syncwarp();
         // ---- item prologue: lane l stages item rows l, l+32, ... and the warp reduces X, Phi
-        const uint4 cv = *reinterpret_cast<const uint4*>(gcnt_ge + g * GQ_GCNT);
         auto rows_ge = [&](uint32_t c) -> int {  // rows of this item among the first c list positions
             return ((int)c > q) ? (int)(((c - q + Q - 1) * rq) >> 16) : 0;
         };
-        // the schedule entries are fetched speculatively (position < 128), in flight together with the counts
+        uint4 cv;
         uint32_t ev[T][4];
+        if (xraw == nullptr) {
+            // the schedule entries are fetched speculatively (position < 128), in flight together with the counts
+            cv = *reinterpret_cast<const uint4*>(gcnt_ge + g * GQ_GCNT);
 #pragma unroll
-        for (int jj = 0; jj < 4; ++jj) {
-            const int pos = q + (lane + 32 * jj) * Q;
+            for (int jj = 0; jj < 4; ++jj) {
+                const int pos = q + (lane + 32 * jj) * Q;
 #pragma unroll
-            for (int t = 0; t < T; ++t) ev[t][jj] = (pos < GQ_G) ? gsched[(size_t)t * K + g * GQ_G + pos] : 0u;
+                for (int t = 0; t < T; ++t) ev[t][jj] = (pos < GQ_G) ? gsched[(size_t)t * K + g * GQ_G + pos] : 0u;
+            }
+        } else {
+            // grinqh_vmm_thresholds: the warp makes the group's schedule itself from x and the thresholds
+            // — widths by comparison, union over tokens, partition128 — in the two ring slots the
+            // item prologue does not fill; no assignment kernel, no schedule in global memory.
+            uint32_t* s_list = reinterpret_cast<uint32_t*>(wbase + C::RING_OFF + (RING - 2) * SLOT_BYTES);
+            uint2 xv[T];
+#pragma unroll
+            for (int t = 0; t < T; ++t) xv[t] = *reinterpret_cast<const uint2*>(xraw + (size_t)t * K + g * GQ_G + 4 * lane);
+            int bt[T][4], bu[4] = {0, 0, 0, 0}, pos[4], ge[10];
+#pragma unroll
+            for (int t = 0; t < T; ++t) {
+                const int m[4] = {(int)(xv[t].x & 0x7FFF), (int)((xv[t].x >> 16) & 0x7FFF), (int)(xv[t].y & 0x7FFF),
+                                  (int)((xv[t].y >> 16) & 0x7FFF)};
+#pragma unroll
+                for (int i = 0; i < 4; ++i) {
+                    int b = 0;
+#pragma unroll
+                    for (int d = 0; d < 8; ++d) b += (m[i] >= tp.thr[d]) ? tp.mult[d] : 0;
+                    bt[t][i] = b;
+                    bu[i] = max(bu[i], b);
+                }
+            }
+            partition128(bu, lane, pos, ge);
+#pragma unroll
+            for (int t = 0; t < T; ++t) {
+                const uint32_t xs[4] = {xv[t].x & 0xFFFFu, xv[t].x >> 16, xv[t].y & 0xFFFFu, xv[t].y >> 16};
+#pragma unroll
+                for (int i = 0; i < 4; ++i)
+                    s_list[t * GQ_G + pos[i]] = (uint32_t)(4 * lane + i) | ((uint32_t)bt[t][i] << 8) |
+                                                ((uint32_t)bu[i] << 12) | (xs[i] << 16);
+            }
+            cv.x = (uint32_t)ge[0] | ((uint32_t)ge[1] << 8) | ((uint32_t)ge[2] << 16) | ((uint32_t)ge[3] << 24);
+            cv.y = (uint32_t)ge[4] | ((uint32_t)ge[5] << 8) | ((uint32_t)ge[6] << 16) | ((uint32_t)ge[7] << 24);
+            cv.z = (uint32_t)ge[8];
+            cv.w = 0;
+            __syncwarp();
+#pragma unroll
+            for (int jj = 0; jj < 4; ++jj) {
+                const int pos_i = q + (lane + 32 * jj) * Q;
+#pragma unroll
+                for (int t = 0; t < T; ++t) ev[t][jj] = (pos_i < GQ_G) ? s_list[t * GQ_G + pos_i] : 0u;
+            }
+            __syncwarp();  // the list is consumed before the ring slots are handed to the copies
         }
         const int n_rows = rows_ge((cv.x >> 8) & 0xFF);
         float X[T], Phi[T];
@@ -442,7 +495,7 @@ constexpr size_t TICKET_BYTES = 16384;  // head of the workspace: one int per co
 template <int T, bool A16, bool FUSED>
 static int launch_main_impl(int K, int N, const VmmPlan& pl, const uint32_t* planes, const void* scales,
                             const void* zeros, const uint32_t* gsched, const uint8_t* gcnt_ge, void* workspace,
-                            float* y, cudaStream_t st) {
+                            float* y, cudaStream_t st, const uint16_t* xraw, const ThrParams& tp) {
     constexpr int smem = Cfg<T>::SMEM;
     static bool configured = false;
     if (!configured) {
@@ -455,18 +508,18 @@ static int launch_main_impl(int K, int N, const VmmPlan& pl, const uint32_t* pla
     const uint32_t rq = (65536u + pl.Q - 1) / pl.Q;
     const cudaError_t e = launch_pdl(vmm_main_kernel<T, A16, FUSED>, grid, dim3(VTHREADS), (size_t)smem, st, K, N, pl.Q, rq,
                                      pl.ipw, pl.Sx, planes, (const __half*)scales, (const __half*)zeros, gsched,
-                                     gcnt_ge, (float*)((char*)workspace + TICKET_BYTES), (int*)workspace, y);
+                                     gcnt_ge, (float*)((char*)workspace + TICKET_BYTES), (int*)workspace, y, xraw, tp);
     return e == cudaSuccess ? GRINQH_OK : GRINQH_ERR_CUDA;
 }
 
 template <bool FUSED>
 static int launch_main(int T, int K, int N, const VmmPlan& pl, const uint32_t* planes, const void* scales,
                        const void* zeros, const uint32_t* gsched, const uint8_t* gcnt_ge, void* ws, float* y,
-                       cudaStream_t st) {
+                       cudaStream_t st, const uint16_t* xraw = nullptr, const ThrParams& tp = ThrParams{}) {
 #define GQ_LAUNCH(TT)                                                                                              \
     return (N % 128 == 0)                                                                                          \
-               ? launch_main_impl<TT, true, FUSED>(K, N, pl, planes, scales, zeros, gsched, gcnt_ge, ws, y, st)    \
-               : launch_main_impl<TT, false, FUSED>(K, N, pl, planes, scales, zeros, gsched, gcnt_ge, ws, y, st)
+               ? launch_main_impl<TT, true, FUSED>(K, N, pl, planes, scales, zeros, gsched, gcnt_ge, ws, y, st, xraw, tp)    \
+               : launch_main_impl<TT, false, FUSED>(K, N, pl, planes, scales, zeros, gsched, gcnt_ge, ws, y, st, xraw, tp)
     switch (T) {
         case 1: GQ_LAUNCH(1);
         case 2: GQ_LAUNCH(2);
@@ -544,4 +597,35 @@ extern "C" int grinqh_vmm_reduce(int T, int K, int N, float* y, const void* work
     gq::vmm_reduce_kernel<<<grid, gq::VTHREADS, 0, (cudaStream_t)stream>>>(
         (const float*)((const char*)workspace + gq::TICKET_BYTES), pl.Sx, T, N, y);
     return cudaGetLastError() == cudaSuccess ? GRINQH_OK : GRINQH_ERR_CUDA;
+}
+
+// SURVEY.md 8f4 (assignment fused into the consumer): the paper's threshold assignment made inside
+// the VMM launch — every warp derives its group's widths and list from x and theta; one launch per projection and
+// no assignment kernel.  y equals grinqh_assign_thresholds + grinqh_vmm bit for bit.
+extern "C" int grinqh_vmm_thresholds(const void* x_f16, int T, int K, int N, int group, const uint16_t theta[9],
+                                     const uint32_t* planes, const void* scales_f16, const void* zeros_f16, float* y,
+                                     void* workspace, size_t workspace_bytes, void* stream) {
+    if (!y || !x_f16 || !theta) return GRINQH_ERR_NULL;
+    if (((uintptr_t)y | (uintptr_t)x_f16) & 15) return GRINQH_ERR_ALIGN;
+    // (the schedule pointers are unused in this mode; pass the planes pointer to satisfy the shared checks)
+    const int rc = gq::check_vmm_ptrs(T, K, N, group, planes, scales_f16, zeros_f16, planes, planes, workspace,
+                                      workspace_bytes);
+    if (rc != GRINQH_OK) return rc;
+    for (int w = 1; w <= 8; ++w)
+        if (theta[w] > 0x8000 || (w > 1 && theta[w] < theta[w - 1])) return GRINQH_ERR_MIX;
+    gq::ThrParams tp;
+    int nd = 0;
+    for (int d = 0; d < 8; ++d) {
+        tp.thr[d] = 0x8000;
+        tp.mult[d] = 0;
+    }
+    for (int w = 1; w <= 8; ++w) {  // distinct reachable thresholds
+        if (theta[w] == 0x8000) continue;
+        int d = 0;
+        while (d < nd && tp.thr[d] != (int)theta[w]) ++d;
+        if (d == nd) tp.thr[nd++] = (int)theta[w];
+        tp.mult[d]++;
+    }
+    return gq::launch_main<true>(T, K, N, gq::vmm_plan(T, K, N), planes, scales_f16, zeros_f16, nullptr, nullptr,
+                                 workspace, y, (cudaStream_t)stream, (const uint16_t*)x_f16, tp);
 }

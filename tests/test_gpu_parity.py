@@ -305,3 +305,25 @@ def test_assign_thresholds_extremes(gq):
         _check_assign(ref, a, x)
     with pytest.raises(gq.GrinqhError):
         gq.grinqh_assign_thresholds(_dev(x), [0, 5, 4, 5, 5, 5, 5, 5, 5])
+
+
+@pytest.mark.parametrize("T,K,N,mix,seed", [(1, 1024, 2048, "4", 0), (2, 2048, 1024 + 96, "3", 1), (4, 512, 4096, "2", 2),
+                                            (1, 4096, 6144, "4", 3), (3, 384, 160, "5", 4)])
+def test_vmm_thresholds_fused_equals_two_calls(gq, T, K, N, mix, seed):
+    """grinqh_vmm_thresholds (assignment inside the VMM launch) == grinqh_assign_thresholds + grinqh_vmm bit for bit,
+    and within tolerance of the oracle's threshold assignment + definitional VMM."""
+    W = synth.make_weights(K, N, 0.02, seed)
+    counts = oracle.mix_to_counts(K, synth.MIXES[mix])
+    xs = np.concatenate([synth.make_x(1, K, 300 + seed * 10 + s, "student_t") for s in range(4)], axis=0)
+    theta = oracle.calibrate_thresholds(xs, counts)
+    x = synth.make_x(T, K, 900 + seed, "student_t")
+    w = gq.grinqh_pack(_dev(W))
+    xd = _dev(x)
+    y_f = gq.grinqh_vmm_thresholds(xd, theta, w).cpu().numpy()
+    a = gq.grinqh_assign_thresholds(xd, theta)
+    y_2 = gq.grinqh_vmm(w, a).cpu().numpy()
+    assert np.array_equal(y_f, y_2)
+    planes, s, z = oracle.pack(W)
+    y_ref = oracle.vmm(x, planes, s, z, oracle.assign_thresholds(x, theta)["bits"])
+    for t in range(T):
+        assert rel_l2(y_f[t], y_ref[t]) <= TOL
