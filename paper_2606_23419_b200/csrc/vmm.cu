@@ -301,8 +301,20 @@ vmm_main_kernel(int K, int N, int Q, uint32_t rq, int ipw, int Sx, const uint32_
             cp_async_commit();
             ++next_v;
         };
+        // lean form when the virtual row is known to be a real row (no scale/zero chunk, no bounds): the common case
+        auto issue_row = [&](auto hi_tag) {
+            issue(next_v, (uint32_t)(next_v & (RING - 1)) * SLOT_BYTES, hi_tag);
+            cp_async_commit();
+            ++next_v;
+        };
+        const int n_lean = max(0, n_rows - (RING - 2));  // rows i < n_lean prefetch a real row (i + RING - 2 < n_rows)
+        if (n_lean > 0) {
 #pragma unroll
-        for (int i = 0; i < RING - 2; ++i) issue_next(HiT{});
+            for (int i = 0; i < RING - 2; ++i) issue_row(HiT{});
+        } else {
+#pragma unroll
+            for (int i = 0; i < RING - 2; ++i) issue_next(HiT{});
+        }
 
         // one row: plane words of its ring slot -> 32 truncated codes -> 32 FMAs per token
         auto consume = [&](auto b_tag, int i) {
@@ -350,22 +362,17 @@ vmm_main_kernel(int K, int N, int Q, uint32_t rq, int ipw, int Sx, const uint32_
             }
         };
 
-        // rows [i0, i1) of the item, all of width B (B = 0: any width, read from the schedule), two per iteration:
-        // one wait + warp barrier, two copies issued into the two slots freed by the previous iteration, then the
-        // two rows' expansion and FMAs are independent instruction streams the scheduler can interleave.
+        // rows [i0, i1) of the item, all of width B (B = 0: any width, read from the schedule)
         auto run = [&](auto b_tag, auto hi_tag, int i0, int i1) {
-            constexpr int PAIR = 1;  // 2 (two independent rows per iteration) was measured: no gain, the loop is not ILP-bound
             int i = i0;
-            for (; i + PAIR <= i1; i += PAIR) {
-                cp_async_wait<RING - 2 - PAIR>();
+            for (const int ie = min(i1, n_lean); i < ie; ++i) {  // steady state: one row in, one row out
+                cp_async_wait<RING - 3>();
                 __syncwarp();
-#pragma unroll
-                for (int u = 0; u < PAIR; ++u) issue_next(hi_tag);
-#pragma unroll
-                for (int u = 0; u < PAIR; ++u) consume(b_tag, i + u);
+                issue_row(hi_tag);
+                consume(b_tag, i);
             }
-            for (; i < i1; ++i) {  // odd tail of a pair run (next_v may run one ahead of a paired schedule: harmless)
-                cp_async_wait<RING - 2 - PAIR>();
+            for (; i < i1; ++i) {  // the item's last RING-2 rows: scale/zero chunks (or nothing) follow the rows
+                cp_async_wait<RING - 3>();
                 __syncwarp();
                 issue_next(hi_tag);
                 consume(b_tag, i);
