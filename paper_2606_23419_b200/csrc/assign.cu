@@ -1,4 +1,5 @@
-// assign.cu — grinqh_assign: |x| ranking -> per-channel bit widths -> compacted row lists (v3).
+// assign.cu — grinqh_assign (rank form) and grinqh_assign_thresholds (the paper's threshold form):
+// |x| -> per-channel bit widths -> compacted row lists.
 // PAPER.md:61-65 (assignment), :271 (top-p partition of the live vector); readings #2-#4.
 //
 // One thread-block cluster of 8 CTAs x 512 threads (8 SMs: a single SM is compute-bound on this, ~400 lane-ops
@@ -15,8 +16,9 @@
 // per 128-row group, then a scan over its groups — no extra cluster barrier).  fp16 has few distinct
 // magnitudes, so splits are the common case, not the exception.
 // Widths: b = sum_d mult_d [key above cut d].  Lists: one warp per 128-row group partitions its rows by
-// (width desc, index asc) with ballots -> grows, gcnt_ge, gsched; a scan over the groups' per-width counts
-// places every group's runs in the global `rows`.
+// (width desc, index asc) with one packed warp scan (partition128) -> grows, gcnt_ge, gsched; a scan over the
+// groups' per-width counts places every group's runs in the global `rows`.  The threshold form skips the select:
+// the cut keys are given.
 #include <cooperative_groups.h>
 
 #include "common.cuh"
