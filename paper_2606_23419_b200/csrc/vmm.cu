@@ -27,7 +27,7 @@
 
 namespace gq {
 
-constexpr int VW = 8;  // warps per CTA
+constexpr int VW = 8;  // warps per CTA (16 in the wide variant: half as many split-K partials, 1 CTA per SM)
 constexpr int VTHREADS = VW * 32;
 constexpr int TILE_COLS = 1024;
 constexpr int SLOT_BYTES = 1024;   // 8 planes x 128 B
@@ -44,7 +44,7 @@ struct Cfg {
     static constexpr int ITEM_OFF = YACC_OFF + T * YSLOT * 4;
     static constexpr int TOK_OFF = ITEM_OFF + 1024;
     static constexpr int WARP_BYTES = TOK_OFF + (T - 1) * 512;
-    static constexpr int SMEM = VW * WARP_BYTES;
+    static constexpr int SMEM = VW * WARP_BYTES;  // x2 for the 16-warp variant
     static_assert(WARP_BYTES % 16 == 0, "warp regions stay 16-byte aligned");
 };
 
@@ -53,27 +53,31 @@ struct VmmPlan {
     int Q;          // sub-chunks per group
     int Sx;         // CTAs (= split-K partials) per column tile
     int ipw;        // items per warp; warp slot ws owns items [ws*ipw, min(I, (ws+1)*ipw)), I = (K/128)*Q
+    int vw;         // warps per CTA: 8 (2 CTAs per SM) or 16 (1 CTA per SM, half the partials)
 };
 
 // Static plan from the shape only (the workspace size depends on it).  Cost model in "rows": a warp does
-// ipw * (rows per item + item overhead); pick the Q in 1..8 that minimises it under the residency limit.
+// ipw * (rows per item + item overhead), and the launch ends with the last CTA's second pass over Sx partials;
+// pick (warps per CTA, Q in 1..8) that minimises the sum under the residency limit (16 warps per SM either way).
 static inline VmmPlan vmm_plan(int T, int K, int N) {
     VmmPlan best{};
     const int CT = (N + TILE_COLS - 1) / TILE_COLS;
     const int groups = K / GQ_G;
-    const int resident = NUM_SMS * ctas_per_sm(T);
-    const int sx_max = resident / CT > 0 ? resident / CT : 1;
     double best_cost = 1e30;
-    for (int Q = 1; Q <= 8; ++Q) {
-        const int I = groups * Q;
-        int Sx = (I + VW - 1) / VW;
-        if (Sx > sx_max) Sx = sx_max;
-        const int ipw = (I + VW * Sx - 1) / (VW * Sx);
-        Sx = (I + VW * ipw - 1) / (VW * ipw);
-        const double cost = ipw * (112.0 / Q + 6.0);
-        if (cost < best_cost - 1e-9) {
-            best_cost = cost;
-            best = VmmPlan{CT, Q, Sx, ipw};
+    for (int vw = 8; vw <= ((T <= 2) ? 16 : 8); vw *= 2) {
+        const int resident = NUM_SMS * (vw == 8 ? ctas_per_sm(T) : 1);
+        const int sx_max = resident / CT > 0 ? resident / CT : 1;
+        for (int Q = 1; Q <= 16; ++Q) {
+            const int I = groups * Q;
+            int Sx = (I + vw - 1) / vw;
+            if (Sx > sx_max) Sx = sx_max;
+            const int ipw = (I + vw * Sx - 1) / (vw * Sx);
+            Sx = (I + vw * ipw - 1) / (vw * ipw);
+            const double cost = ipw * (112.0 / Q + 6.0) + 4.0 + 0.12 * Sx;  // + second pass, in row units (~0.45 us)
+            if (cost < best_cost - 1e-9) {
+                best_cost = cost;
+                best = VmmPlan{CT, Q, Sx, ipw, vw};
+            }
         }
     }
     return best;
@@ -120,8 +124,8 @@ __device__ __forceinline__ void accumulate_row(const uint32_t (&V)[8], uint16_t 
 //
 // FUSED: the last CTA of a column tile to finish (ticket counter in the workspace, reset to 0 by that CTA) sums the
 // tile's Sx partials in the fixed order s = 0..Sx-1 and writes y: still deterministic, one launch instead of two.
-template <int T, bool A16, bool FUSED>
-__global__ void __launch_bounds__(VTHREADS, ctas_per_sm(T))
+template <int T, int VWT, bool A16, bool FUSED>
+__global__ void __launch_bounds__(VWT * 32, VWT == 8 ? ctas_per_sm(T) : 1)
 vmm_main_kernel(int K, int N, int Q, uint32_t rq, int ipw, int Sx, const uint32_t* __restrict__ planes,
                 const __half* __restrict__ scales, const __half* __restrict__ zeros,
                 const uint32_t* __restrict__ gsched, const uint8_t* __restrict__ gcnt_ge,
@@ -159,7 +163,7 @@ vmm_main_kernel(int K, int N, int Q, uint32_t rq, int ipw, int Sx, const uint32_
     pdl_launch_dependents();
     pdl_wait();  // nothing global (schedule, partials, tickets) is touched before the previous kernel has finished
 
-    const int ws = sx * VW + warp;
+    const int ws = sx * VWT + warp;
     const int it0 = ws * ipw;
     const int it1 = min(I, it0 + ipw);
     bool first = true;
@@ -439,14 +443,14 @@ vmm_main_kernel(int K, int N, int Q, uint32_t rq, int ipw, int Sx, const uint32_
 #pragma unroll
     for (int t = 0; t < T; ++t)
 #pragma unroll
-        for (int i = 0; i < TILE_COLS / VTHREADS; ++i) {
-            const int c = tid + VTHREADS * i;  // column inside the tile
+        for (int i = 0; i < TILE_COLS / (VWT * 32); ++i) {
+            const int c = tid + VWT * 32 * i;  // column inside the tile
             const int n = tile * TILE_COLS + c;
             if (n < N) {
                 const int idx = (c & 31) * 33 + (c >> 5);
                 float A = 0.f;
 #pragma unroll
-                for (int w = 0; w < VW; ++w)
+                for (int w = 0; w < VWT; ++w)
                     A += *reinterpret_cast<const float*>(smem + w * C::WARP_BYTES + C::YACC_OFF + (t * YSLOT + idx) * 4);
                 out[(size_t)t * N + n] = A;
             }
@@ -459,8 +463,8 @@ vmm_main_kernel(int K, int N, int Q, uint32_t rq, int ipw, int Sx, const uint32_
         __syncthreads();
         if (s_last) {
             __threadfence();
-            const int n = tile * TILE_COLS + 4 * tid;  // 4 columns per thread
-            if (n < N) {
+            const int n = tile * TILE_COLS + 4 * tid;  // 4 columns per thread (the first 256 threads)
+            if (4 * tid < TILE_COLS && n < N) {
 #pragma unroll
                 for (int t = 0; t < T; ++t) {
                     float4 a = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -499,23 +503,24 @@ vmm_reduce_kernel(const float* __restrict__ part, int S, int T, int N, float* __
 
 constexpr size_t TICKET_BYTES = 16384;  // head of the workspace: one int per column tile, zero between launches
 
-template <int T, bool A16, bool FUSED>
+template <int T, int VWT, bool A16, bool FUSED>
 static int launch_main_impl(int K, int N, const VmmPlan& pl, const uint32_t* planes, const void* scales,
                             const void* zeros, const uint32_t* gsched, const uint8_t* gcnt_ge, void* workspace,
                             float* y, cudaStream_t st, const uint16_t* xraw, const ThrParams& tp) {
-    constexpr int smem = Cfg<T>::SMEM;
+    constexpr int smem = Cfg<T>::WARP_BYTES * VWT;
     static bool configured = false;
     if (!configured) {
-        if (cudaFuncSetAttribute(vmm_main_kernel<T, A16, FUSED>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) !=
-            cudaSuccess)
+        if (cudaFuncSetAttribute(vmm_main_kernel<T, VWT, A16, FUSED>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 smem) != cudaSuccess)
             return GRINQH_ERR_CUDA;
         configured = true;
     }
     dim3 grid(pl.col_tiles, pl.Sx);
     const uint32_t rq = (65536u + pl.Q - 1) / pl.Q;
-    const cudaError_t e = launch_pdl(vmm_main_kernel<T, A16, FUSED>, grid, dim3(VTHREADS), (size_t)smem, st, K, N, pl.Q, rq,
-                                     pl.ipw, pl.Sx, planes, (const __half*)scales, (const __half*)zeros, gsched,
-                                     gcnt_ge, (float*)((char*)workspace + TICKET_BYTES), (int*)workspace, y, xraw, tp);
+    const cudaError_t e = launch_pdl(vmm_main_kernel<T, VWT, A16, FUSED>, grid, dim3(VWT * 32), (size_t)smem, st, K, N,
+                                     pl.Q, rq, pl.ipw, pl.Sx, planes, (const __half*)scales, (const __half*)zeros,
+                                     gsched, gcnt_ge, (float*)((char*)workspace + TICKET_BYTES), (int*)workspace, y,
+                                     xraw, tp);
     return e == cudaSuccess ? GRINQH_OK : GRINQH_ERR_CUDA;
 }
 
@@ -523,16 +528,22 @@ template <bool FUSED>
 static int launch_main(int T, int K, int N, const VmmPlan& pl, const uint32_t* planes, const void* scales,
                        const void* zeros, const uint32_t* gsched, const uint8_t* gcnt_ge, void* ws, float* y,
                        cudaStream_t st, const uint16_t* xraw = nullptr, const ThrParams& tp = ThrParams{}) {
-#define GQ_LAUNCH(TT)                                                                                              \
-    return (N % 128 == 0)                                                                                          \
-               ? launch_main_impl<TT, true, FUSED>(K, N, pl, planes, scales, zeros, gsched, gcnt_ge, ws, y, st, xraw, tp)    \
-               : launch_main_impl<TT, false, FUSED>(K, N, pl, planes, scales, zeros, gsched, gcnt_ge, ws, y, st, xraw, tp)
+#define GQ_LAUNCH_W(TT, WW)                                                                                              \
+    return (N % 128 == 0)                                                                                                \
+               ? launch_main_impl<TT, WW, true, FUSED>(K, N, pl, planes, scales, zeros, gsched, gcnt_ge, ws, y, st, xraw, tp) \
+               : launch_main_impl<TT, WW, false, FUSED>(K, N, pl, planes, scales, zeros, gsched, gcnt_ge, ws, y, st, xraw, tp)
+    if (pl.vw == 16) {  // only planned for T <= 2 (registers)
+        if (T == 1) { GQ_LAUNCH_W(1, 16); }
+        GQ_LAUNCH_W(2, 16);
+    }
+#define GQ_LAUNCH(TT) GQ_LAUNCH_W(TT, 8)
     switch (T) {
         case 1: GQ_LAUNCH(1);
         case 2: GQ_LAUNCH(2);
         case 3: GQ_LAUNCH(3);
         default: GQ_LAUNCH(4);
     }
+#undef GQ_LAUNCH_W
 #undef GQ_LAUNCH
 }
 
