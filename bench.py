@@ -25,8 +25,8 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
 # DRAM bytes moved by the 4 VMM launches of one step, from the committed ncu --set full capture (profiles/r01_kernels.md):
-# 116.24 MB read + 0.82 MB written, against 116.23 MB algorithmic.  Only the default mix was captured.
-NCU_TRAFFIC_BYTES_PER_STEP = {"4": 117.06e6}
+# 116.26 MB read + 0.67 MB written, against 116.23 MB algorithmic.  Only the default mix was captured.
+NCU_TRAFFIC_BYTES_PER_STEP = {"4": 116.94e6}
 METRIC = "us per decode step of one Llama-3-8B-shaped layer (4 assigns + the 7 projections as bit-planar VMMs), batch 1"
 UNIT = "us"
 
@@ -406,7 +406,7 @@ def run_native(args):
                      "traffic": NCU_TRAFFIC_BYTES_PER_STEP.get(args.mix),
                      "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum over the step's VMM launches, "
                                        "ncu --set full capture of this command (profiles/r01_kernels.md)",
-                     "kernel": f"vmm_main_kernel<1,1,1> ({len(fused)} launches per step)",
+                     "kernel": f"vmm_main_kernel<T=1, 16 warps, 16-byte copies, fused second pass> ({len(fused)} launches per step)",
                      "alg_bytes_per_step": step_bytes, "plane_bytes_per_step": plane_bytes,
                      "us_per_step_main_only": us_main, "peak_source": peak_src},
         "pack": {"GBps": pack_bytes / (pack_ms * 1e-3) / 1e9, "ms_per_layer": pack_ms / L},
