@@ -42,6 +42,7 @@ def _args():
     ap.add_argument("--seed", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sweep", action="store_true", help="configs 3 and 5: per-VMM latency vs average bits (not the contract line)")
+    ap.add_argument("--prefill", action="store_true", help="f3 (part): grinqh_unpack + dense library GEMM timings")
     ap.add_argument("--decode-step", action="store_true", help="config 4: 32-layer decode step in one CUDA graph")
     ap.add_argument("--no-split", action="store_true", help="skip the one-launch-per-projection variant")
     return ap.parse_args()
@@ -607,9 +608,54 @@ def run_decode_step(args):
                                       "frac_of_measured_hbm": nbytes / us / 1e3 / peak}), flush=True)
 
 
+# ------------------------------------------------------------------------------------------ prefill half (f3)
+def run_prefill(args):
+    """SURVEY.md 8f3 / PAPER.md:101: unpack at b_max (grinqh_unpack), then a dense library GEMM on the result.
+    One JSON line per shape, prefixed "PREFILL "."""
+    import torch
+
+    from paper_2606_23419_b200 import binding as gq
+
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    peak, _ = _peaks()
+    gen = torch.Generator(device=dev)
+    gen.manual_seed(args.seed)
+    tokens = 3000                                       # the paper's 3000:1 prefill benchmark (PAPER.md:158-166)
+    for K, N in [(4096, 14336), (14336, 4096), (8192, 28672)]:
+        W = (torch.randn((K, N), generator=gen, device=dev) * 0.02).half()
+        w = gq.grinqh_pack(W)
+        out = torch.empty_like(W)
+        X = torch.randn((tokens, K), device=dev, dtype=torch.float16)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+
+        def timed(fn, reps):
+            for _ in range(3):
+                fn()
+            torch.cuda.synchronize()
+            a.record()
+            for _ in range(reps):
+                fn()
+            b.record()
+            torch.cuda.synchronize()
+            return a.elapsed_time(b) * 1e3 / reps
+
+        us_unpack = timed(lambda: gq.grinqh_unpack(w, out), 20)
+        us_gemm = timed(lambda: torch.matmul(X, out), 10)
+        print("PREFILL " + json.dumps({"K": K, "N": N, "tokens": tokens, "us_unpack": us_unpack,
+                                       "unpack_GBps": K * N * 3 / us_unpack / 1e3,
+                                       "unpack_frac_of_measured_hbm": K * N * 3 / us_unpack / 1e3 / peak,
+                                       "us_dense_gemm_fp16_torch": us_gemm,
+                                       "gemm_TFLOPs": 2 * tokens * K * N / us_gemm / 1e6,
+                                       "unpack_over_gemm": us_unpack / us_gemm}), flush=True)
+        del W, w, out, X
+
+
 def main():
     args = _args()
-    if args.decode_step:
+    if args.prefill:
+        run_prefill(args)
+    elif args.decode_step:
         run_decode_step(args)
     elif args.sweep:
         run_sweep(args)

@@ -90,6 +90,16 @@ int grinqh_pack(const void* W_f16, int K, int N, int group,
                 uint32_t* planes, void* scales_f16, void* zeros_f16, void* stream);
 
 /*
+ * grinqh_unpack — the first half of the paper's prefill path ("unpack at b_max, dense GEMM";
+ * stage decoupling :51).  Rebuilds the full 8-bit codes from the 8 planes and writes W_hat = s * q + z as fp16: the
+ * fp64 value rounded once (round-to-nearest-even).  The dense GEMM that follows is an ordinary library GEMM on W_f16.
+ *   planes, scales_f16, zeros_f16   dev   as written by grinqh_pack
+ *   W_f16      dev  [K, N] fp16, written
+ */
+int grinqh_unpack(const uint32_t* planes, const void* scales_f16, const void* zeros_f16, int K, int N, int group,
+                  void* W_f16, void* stream);
+
+/*
  * grinqh_assign — every decode step, once per input vector
  * (PAPER.md:61-65 assignment, :271 top-p partition of the live vector).
  * Per token t: order channels by (|x_tk| descending, k ascending) on the 15

@@ -33,6 +33,8 @@ _lib.grinqh_mix_to_counts.restype = _i
 _lib.grinqh_mix_to_counts.argtypes = [_i, _vp, _vp]
 _lib.grinqh_pack.restype = _i
 _lib.grinqh_pack.argtypes = [_vp, _i, _i, _i, _vp, _vp, _vp, _vp]
+_lib.grinqh_unpack.restype = _i
+_lib.grinqh_unpack.argtypes = [_vp, _vp, _vp, _i, _i, _i, _vp, _vp]
 _lib.grinqh_assign_workspace_bytes.restype = _sz
 _lib.grinqh_assign_workspace_bytes.argtypes = [_i, _i]
 _lib.grinqh_assign.restype = _i
@@ -58,7 +60,7 @@ _lib.grinqh_decode_host.restype = _i
 _lib.grinqh_decode_host.argtypes = [_vp, _i, _i, _i, _i, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp,
                                     _vp, _vp, _sz, _vp, _vp, _sz, _vp, _i, _vp]
 
-EXPORTS = ("grinqh_status_string", "grinqh_version", "grinqh_mix_to_counts", "grinqh_pack",
+EXPORTS = ("grinqh_status_string", "grinqh_version", "grinqh_mix_to_counts", "grinqh_pack", "grinqh_unpack",
            "grinqh_assign_workspace_bytes", "grinqh_assign", "grinqh_assign_thresholds",
            "grinqh_calibrate_thresholds", "grinqh_vmm_workspace_bytes",
            "grinqh_vmm_workspace_init", "grinqh_vmm", "grinqh_vmm_thresholds",
@@ -120,6 +122,15 @@ def grinqh_pack(W: torch.Tensor, out: Packed | None = None, stream=None) -> Pack
     out = out or Packed(K, N, W.device)
     _check(_lib.grinqh_pack(_dev(W, torch.float16, "W"), K, N, GROUP, out.planes.data_ptr(),
                             out.scales.data_ptr(), out.zeros.data_ptr(), _stream(stream)), "grinqh_pack")
+    return out
+
+
+def grinqh_unpack(w: Packed, out: torch.Tensor | None = None, stream=None) -> torch.Tensor:
+    """Full-precision dequantised weights [K, N] fp16 (prefill path: unpack at b_max, then a dense GEMM)."""
+    if out is None:
+        out = torch.empty((w.K, w.N), dtype=torch.float16, device=w.planes.device)
+    _check(_lib.grinqh_unpack(w.planes.data_ptr(), w.scales.data_ptr(), w.zeros.data_ptr(), w.K, w.N, GROUP,
+                              _dev(out, torch.float16, "W"), _stream(stream)), "grinqh_unpack")
     return out
 
 

@@ -327,3 +327,21 @@ def test_vmm_thresholds_fused_equals_two_calls(gq, T, K, N, mix, seed):
     y_ref = oracle.vmm(x, planes, s, z, oracle.assign_thresholds(x, theta)["bits"])
     for t in range(T):
         assert rel_l2(y_f[t], y_ref[t]) <= TOL
+
+
+@pytest.mark.parametrize("K,N,std,seed", [(256, 512, 0.02, 0), (384, 1056, 0.02, 1), (128, 32, 1.0, 3), (1024, 4096, 0.015, 4)])
+def test_unpack_is_the_correctly_rounded_full_precision_dequant(gq, K, N, std, seed):
+    """SURVEY.md 8f3 (first half of the prefill path): planes -> fp16 W_hat, bit-exact against the oracle's
+    fp64 dequantisation rounded once to fp16; and the dense product on it matches the all-8-bit VMM."""
+    W = synth.make_weights(K, N, std, seed)
+    W[:128, 0] = np.float16(0.25)                      # a constant group (s = 0)
+    w = gq.grinqh_pack(_dev(W))
+    Wh = gq.grinqh_unpack(w)
+    torch.cuda.synchronize()
+    planes, s, z = oracle.pack(W)
+    ref = oracle.dequant(planes, s, z, 8).astype(np.float16)
+    assert np.array_equal(Wh.cpu().numpy().view(np.uint16), ref.view(np.uint16))
+    x = synth.make_x(3, K, seed + 50)
+    y_dense = (torch.from_numpy(x).cuda().float() @ Wh.float()).cpu().numpy()   # prefill-style dense product
+    y_ref = x.astype(np.float64) @ oracle.dequant(planes, s, z, 8)
+    assert rel_l2(y_dense, y_ref) <= 2e-3              # fp16 W_hat: rounding of the weights themselves (2^-11 relative)
