@@ -133,7 +133,6 @@ vmm_main_kernel(int K, int N, int Q, uint32_t rq, int ipw, int Sx, const uint32_
                 const uint16_t* __restrict__ xraw, ThrParams tp) {
     using C = Cfg<T>;
     constexpr int RING = C::RING;
-    constexpr uint32_t RING_MASK = RING * SLOT_BYTES - 1;
     extern __shared__ __align__(16) uint8_t smem[];
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
