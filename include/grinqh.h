@@ -186,10 +186,10 @@ int grinqh_vmm_thresholds(const void* x_f16, int T, int K, int N, int group, con
                           float* y, void* workspace, size_t workspace_bytes, void* stream);
 
 /*
- * Host-buffer decode call (the end-to-end entry): copies x from HOST memory to
- * the device staging buffer x_dev_f16, runs grinqh_assign + grinqh_vmm, and
- * copies y back to HOST memory, all enqueued on `stream` (cudaMemcpyAsync;
- * pass pinned host memory for real asynchrony).  The packed weights stay
+ * Host-buffer decode call (the end-to-end entry): x comes from HOST memory, grinqh_assign + grinqh_vmm run, y ends
+ * in HOST memory, all enqueued on `stream`.  With pinned (page-locked) buffers the kernels access host memory
+ * directly (x is read once by the assignment, y is written by the VMM's second pass): no copy nodes.  With pageable
+ * buffers, or GRINQH_FORCE_COPIES, x is staged through x_dev_f16 and y through y_dev with cudaMemcpyAsync.  The packed weights stay
  * resident on the device.  The caller synchronises the stream before reading
  * y_host.
  *   x_host_f16  HOST [T, K] fp16       y_host  HOST [T, N] fp32
@@ -200,6 +200,7 @@ int grinqh_vmm_thresholds(const void* x_f16, int T, int K, int N, int group, con
  *               skip the host->device copy and grinqh_assign.
  */
 #define GRINQH_REUSE_ASSIGNMENT 1
+#define GRINQH_FORCE_COPIES 2   /* always stage through x_dev_f16 / y_dev with cudaMemcpyAsync */
 int grinqh_decode_host(const void* x_host_f16, int T, int K, int N, int group,
                        const uint32_t counts[9],
                        const uint32_t* planes, const void* scales_f16, const void* zeros_f16,

@@ -246,7 +246,7 @@ def grinqh_vmm_reduce(T: int, K: int, N: int, y: torch.Tensor, workspace: torch.
 
 def grinqh_decode_host(x_host: torch.Tensor, counts, w: Packed, a: Assignment, x_dev: torch.Tensor,
                        y_dev: torch.Tensor, workspace: torch.Tensor, y_host: torch.Tensor,
-                       reuse_assignment: bool = False, stream=None):
+                       reuse_assignment: bool = False, force_copies: bool = False, stream=None):
     """HOST x [T, K] fp16 (pinned) -> HOST y [T, N] fp32 (pinned); weights stay on the device.  Enqueue only."""
     T, K = x_host.shape
     if x_host.is_cuda or y_host.is_cuda:
@@ -256,4 +256,4 @@ def grinqh_decode_host(x_host: torch.Tensor, counts, w: Packed, a: Assignment, x
         w.zeros.data_ptr(), x_dev.data_ptr(), a.bits.data_ptr(), a.bits_union.data_ptr(), a.rows.data_ptr(),
         a.cnt_ge.data_ptr(), a.grows.data_ptr(), a.gcnt_ge.data_ptr(), a.gsched.data_ptr(), None, 0, y_dev.data_ptr(),
         workspace.data_ptr(), workspace.numel() * workspace.element_size(), y_host.data_ptr(),
-        1 if reuse_assignment else 0, _stream(stream)), "grinqh_decode_host")
+        (1 if reuse_assignment else 0) | (2 if force_copies else 0), _stream(stream)), "grinqh_decode_host")

@@ -97,17 +97,35 @@ extern "C" int grinqh_decode_host(const void* x_host_f16, int T, int K, int N, i
     if (vmm_ws_bytes < grinqh_vmm_workspace_bytes(T, K, N)) return GRINQH_ERR_WORKSPACE;
     cudaStream_t st = (cudaStream_t)stream;
     int rc = GRINQH_OK;
+    // Pinned (page-locked) host buffers are visible to the device under unified addressing: the assignment kernel
+    // then reads x straight from host memory (8-57 KB, once) and the VMM's second pass writes y straight into it —
+    // no copy nodes, no staging.  Pageable buffers (or GRINQH_FORCE_COPIES) go through cudaMemcpyAsync + staging.
+    auto device_view = [&](const void* host) -> void* {
+        if (flags & GRINQH_FORCE_COPIES) return nullptr;
+        cudaPointerAttributes a;
+        if (cudaPointerGetAttributes(&a, host) != cudaSuccess) {
+            (void)cudaGetLastError();
+            return nullptr;
+        }
+        return (a.type == cudaMemoryTypeHost && a.devicePointer && !((uintptr_t)a.devicePointer & 15)) ? a.devicePointer
+                                                                                                     : nullptr;
+    };
     if (!(flags & GRINQH_REUSE_ASSIGNMENT)) {
-        if (cudaMemcpyAsync(x_dev_f16, x_host_f16, (size_t)T * K * 2, cudaMemcpyHostToDevice, st) != cudaSuccess)
-            return GRINQH_ERR_CUDA;
-        rc = grinqh_assign(x_dev_f16, T, K, counts, bits, bits_union, rows, cnt_ge, grows, gcnt_ge, gsched,
-                           assign_ws, assign_ws_bytes, stream);
+        const void* xv = device_view(x_host_f16);
+        if (!xv) {
+            if (cudaMemcpyAsync(x_dev_f16, x_host_f16, (size_t)T * K * 2, cudaMemcpyHostToDevice, st) != cudaSuccess)
+                return GRINQH_ERR_CUDA;
+            xv = x_dev_f16;
+        }
+        rc = grinqh_assign(xv, T, K, counts, bits, bits_union, rows, cnt_ge, grows, gcnt_ge, gsched, assign_ws,
+                           assign_ws_bytes, stream);
         if (rc != GRINQH_OK) return rc;
     }
-    rc = grinqh_vmm(T, K, N, group, planes, scales_f16, zeros_f16, gsched, gcnt_ge, y_dev, vmm_ws, vmm_ws_bytes,
-                    stream);
+    float* yv = (float*)device_view(y_host);
+    rc = grinqh_vmm(T, K, N, group, planes, scales_f16, zeros_f16, gsched, gcnt_ge, yv ? yv : y_dev, vmm_ws,
+                    vmm_ws_bytes, stream);
     if (rc != GRINQH_OK) return rc;
-    if (cudaMemcpyAsync(y_host, y_dev, (size_t)T * N * 4, cudaMemcpyDeviceToHost, st) != cudaSuccess)
+    if (!yv && cudaMemcpyAsync(y_host, y_dev, (size_t)T * N * 4, cudaMemcpyDeviceToHost, st) != cudaSuccess)
         return GRINQH_ERR_CUDA;
     return GRINQH_OK;
 }

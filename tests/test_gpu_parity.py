@@ -229,9 +229,18 @@ def test_decode_host_entry(gq):
     xd = torch.empty((1, K), dtype=torch.float16, device="cuda")
     yd = torch.empty((1, N), dtype=torch.float32, device="cuda")
     ws = gq.grinqh_vmm_workspace(1, K, N)
-    gq.grinqh_decode_host(xh, counts, w, a, xd, yd, ws, yh)
+    gq.grinqh_decode_host(xh, counts, w, a, xd, yd, ws, yh)           # pinned: kernels access host memory directly
     torch.cuda.synchronize()
     assert rel_l2(yh.numpy(), y_ref) <= TOL
+    y_direct = yh.numpy().copy()
+    yh.zero_()
+    gq.grinqh_decode_host(xh, counts, w, a, xd, yd, ws, yh, force_copies=True)   # staged with cudaMemcpyAsync
+    torch.cuda.synchronize()
+    assert np.array_equal(yh.numpy(), y_direct)
+    xp, yp = torch.from_numpy(x.copy()), torch.zeros((1, N), dtype=torch.float32)   # pageable host buffers
+    gq.grinqh_decode_host(xp, counts, w, a, xd, yd, ws, yp)
+    torch.cuda.synchronize()
+    assert np.array_equal(yp.numpy(), y_direct)
 
 
 def test_fused_second_pass_matches_two_launches_and_workspace_is_reusable(gq):
