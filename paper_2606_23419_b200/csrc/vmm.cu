@@ -456,12 +456,15 @@ vmm_main_kernel(int K, int N, int Q, uint32_t rq, int ipw, int Sx, const uint32_
         }
     if (FUSED && Sx > 1) {
         __shared__ int s_last;
-        __threadfence();  // this CTA's partial is visible device-wide before its ticket
-        __syncthreads();
-        if (tid == 0) s_last = (atomicAdd(&tickets[tile], 1) == Sx - 1);
+        __syncthreads();  // the CTA's partial is complete ...
+        if (tid == 0) {
+            __threadfence();  // ... and (fence cumulativity over the barrier) visible device-wide before its ticket
+            const int last = (atomicAdd(&tickets[tile], 1) == Sx - 1);
+            if (last) __threadfence();  // acquire side: the other CTAs' partials, read below with ld.global.cg
+            s_last = last;
+        }
         __syncthreads();
         if (s_last) {
-            __threadfence();
             const int n = tile * TILE_COLS + 4 * tid;  // 4 columns per thread (the first 256 threads)
             if (4 * tid < TILE_COLS && n < N) {
 #pragma unroll
