@@ -28,7 +28,7 @@
  *     nothing has been enqueued.
  *   - W is [K, N] row-major fp16: K = d_in rows (input channels), N = d_out.
  *     group = 128 consecutive input channels of one output column
- *     ("group size G=128").  Required: K % 128 == 0, N % 32 == 0,
+ *     ("group size G=128").  Required: K % 128 == 0, K <= 32768, N % 32 == 0,
  *     1 <= T <= 4, all base pointers 16-byte aligned.
  *   - Plane j (j = 0 is the MSB, code bit 7) is planes[j][k][n >> 5], column n
  *     sits at bit (n & 31) of that word.  planes is one allocation of

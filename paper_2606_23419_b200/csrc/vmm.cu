@@ -550,7 +550,8 @@ static int launch_main(int T, int K, int N, const VmmPlan& pl, const uint32_t* p
 }
 
 static int check_vmm_args(int T, int K, int N, int group) {
-    if (group != GQ_G || T < 1 || T > GRINQH_MAX_T || K <= 0 || N <= 0 || K % GQ_G || N % 32) return GRINQH_ERR_SHAPE;
+    if (group != GQ_G || T < 1 || T > GRINQH_MAX_T || K <= 0 || N <= 0 || K % GQ_G || N % 32 || K > GQ_MAX_K)
+        return GRINQH_ERR_SHAPE;  // (K <= 32768 as for grinqh_assign: the item arithmetic assumes <= 4096 items per tile)
     if ((size_t)((N + TILE_COLS - 1) / TILE_COLS) * sizeof(int) > TICKET_BYTES) return GRINQH_ERR_SHAPE;
     return GRINQH_OK;
 }

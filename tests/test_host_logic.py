@@ -70,6 +70,7 @@ def test_argument_validation_without_gpu(lib):
     lib.grinqh_vmm_workspace_bytes.argtypes = [C.c_int] * 3
     assert lib.grinqh_vmm_workspace_bytes(1, 4096, 4096) > 0
     assert lib.grinqh_vmm_workspace_bytes(1, 4000, 4096) == 0
+    assert lib.grinqh_vmm_workspace_bytes(1, 32768, 4096) > 0 and lib.grinqh_vmm_workspace_bytes(1, 32768 + 128, 4096) == 0
     lib.grinqh_vmm.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int] + [vp] * 5 + [vp, vp, C.c_size_t, vp]
     assert lib.grinqh_vmm(1, 128, 32, 128, 16, 16, 16, 16, 16, 16, 16, 0, None) == -5  # workspace
 
