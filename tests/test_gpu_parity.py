@@ -184,10 +184,10 @@ def test_vmm_one_hot_and_determinism(gq):
     assert np.array_equal(y1, y2)                   # deterministic split-K
 
 
-def test_full_size_layer_sampled_columns(gq):
-    """BASELINE.json config 2 shape 4096 -> 14336 in the launch configuration bench.py times;
-    the oracle recomputes a sample of output columns one by one (columns are independent)."""
-    K, N = 4096, 14336
+@pytest.mark.parametrize("K,N", [(4096, 6144), (4096, 4096), (4096, 28672), (14336, 4096), (4096, 14336)])
+def test_full_size_layer_sampled_columns(gq, K, N):
+    """BASELINE.json config 2 at full size, in the launch configurations bench.py times (q|k|v, o, gate|up, down, and a
+    single gate projection); the oracle recomputes a sample of output columns one by one (columns are independent)."""
     g = torch.Generator(device="cuda")
     g.manual_seed(1234)
     Wd = (torch.randn((K, N), generator=g, device="cuda", dtype=torch.float32) * 0.02).to(torch.float16)
@@ -213,6 +213,11 @@ def test_full_size_layer_sampled_columns(gq):
     sub_cols = np.array([remap[int(c) // 32] * 32 + int(c) % 32 for c in cols], np.int32)
     y_ref = oracle.vmm(x, planes, s, z, ref_a["bits"], cols=sub_cols)
     assert rel_l2(y.cpu().numpy()[0, cols], y_ref[0]) <= TOL
+    # the threshold form made inside the VMM launch, same shape
+    theta = oracle.calibrate_thresholds(x, counts)
+    y_t = gq.grinqh_vmm_thresholds(xd, theta, w)
+    y_t_ref = oracle.vmm(x, planes, s, z, oracle.assign_thresholds(x, theta)["bits"], cols=sub_cols)
+    assert rel_l2(y_t.cpu().numpy()[0, cols], y_t_ref[0]) <= TOL
 
 
 def test_decode_host_entry(gq):
