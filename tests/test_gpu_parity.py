@@ -359,3 +359,50 @@ def test_unpack_is_the_correctly_rounded_full_precision_dequant(gq, K, N, std, s
     y_dense = (torch.from_numpy(x).cuda().float() @ Wh.float()).cpu().numpy()   # prefill-style dense product
     y_ref = x.astype(np.float64) @ oracle.dequant(planes, s, z, 8)
     assert rel_l2(y_dense, y_ref) <= 2e-3              # fp16 W_hat: rounding of the weights themselves (2^-11 relative)
+
+
+def test_fuzz_random_shapes_mixes_and_ties(gq):
+    """Randomised sweep (fixed seed): any widths 0..8 with arbitrary counts, 1..4 tokens, ragged N, inputs with many
+    tied magnitudes; rank and threshold forms, two-call and fused VMM.  Integer outputs bit-exact, y within tolerance."""
+    rng = np.random.default_rng(20261104)
+    for case in range(36):
+        T = int(rng.integers(1, 5))
+        K = 128 * int(rng.integers(1, 17))
+        N = 32 * int(rng.integers(1, 41))
+        cuts = np.sort(rng.integers(0, K + 1, 8))
+        counts = np.diff(np.concatenate([[0], cuts, [K]])).astype(np.uint32)
+        rng.shuffle(counts)
+        kind = case % 3
+        if kind == 0:
+            x = synth.make_x(T, K, 1000 + case, "student_t")
+        elif kind == 1:                                   # few distinct magnitudes: every cut splits a tie run
+            x = (rng.integers(-6, 7, (T, K)) * 0.25).astype(np.float16)
+        else:                                             # mostly zeros and a heavy tail
+            x = (rng.standard_t(2.0, (T, K)) * (rng.random((T, K)) < 0.3)).astype(np.float16)
+        W = synth.make_weights(K, N, 0.02, 2000 + case)
+        planes, s, z = oracle.pack(W)
+        w = gq.grinqh_pack(_dev(W))
+        xd = _dev(x)
+        ref = oracle.assign(x, counts)
+        a = gq.grinqh_assign(xd, counts)
+        torch.cuda.synchronize()
+        _check_assign(ref, a, x)
+        y = gq.grinqh_vmm(w, a).cpu().numpy()
+        y_ref = oracle.vmm(x, planes, s, z, ref["bits"])
+        for t in range(T):
+            n = np.linalg.norm(y_ref[t])
+            assert np.linalg.norm(y[t] - y_ref[t]) <= TOL * n + 1e-6, (case, T, K, N, list(counts))
+        theta = np.sort(rng.integers(0, 0x4800, 9)).astype(np.uint16)
+        theta[rng.integers(1, 9):] = 0x8000 if case % 4 == 0 else theta[-1]
+        theta = np.sort(theta)
+        ref_t = oracle.assign_thresholds(x, theta)
+        a_t = gq.grinqh_assign_thresholds(xd, theta)
+        torch.cuda.synchronize()
+        _check_assign(ref_t, a_t, x)
+        y2 = gq.grinqh_vmm(w, a_t).cpu().numpy()
+        y3 = gq.grinqh_vmm_thresholds(xd, theta, w).cpu().numpy()
+        assert np.array_equal(y2, y3), (case, T, K, N)
+        y_ref_t = oracle.vmm(x, planes, s, z, ref_t["bits"])
+        for t in range(T):
+            n = np.linalg.norm(y_ref_t[t])
+            assert np.linalg.norm(y2[t] - y_ref_t[t]) <= TOL * n + 1e-6, (case, T, K, N)
