@@ -345,7 +345,7 @@ vmm_main_kernel(int K, int N, int Q, uint32_t rq, int ipw, int Sx, const uint32_
             }
             if (T == 1) {
                 accumulate_row(V, (uint16_t)(m >> 16), acc[0]);
-            } else {
+            } else if (T == 2) {
                 const int b = (m >> 12) & 15;
 #pragma unroll
                 for (int t = 0; t < T; ++t) {
@@ -360,6 +360,33 @@ vmm_main_kernel(int K, int N, int Q, uint32_t rq, int ipw, int Sx, const uint32_
 #pragma unroll
                         for (int j = 0; j < 8; ++j) Vm[j] = V[j] & mask;
                         accumulate_row(Vm, (uint16_t)(e >> 16), acc[t]);
+                    }
+                }
+            } else {
+                // 3 or 4 tokens: the bytes are widened to fp16 lanes once per row; a token narrower than the union
+                // masks the 16-bit lanes instead of the bytes (no further byte permutes): -12 % at T = 4 (at T = 2 the
+                // 16 extra registers spill, so it keeps the byte form)
+                const int b = (m >> 12) & 15;
+                uint32_t H[16];
+#pragma unroll
+                for (int r = 0; r < 8; ++r) {
+                    H[2 * r] = __byte_perm(V[r], 0u, 0x4140);
+                    H[2 * r + 1] = __byte_perm(V[r], 0u, 0x4342);
+                }
+#pragma unroll
+                for (int t = 0; t < T; ++t) {
+                    const uint32_t e = (t == 0) ? m : s_tok[(t - 1) * GQ_G + i];
+                    const int bt = (e >> 8) & 15;
+                    if (bt == 0) continue;
+                    const uint16_t xh = (uint16_t)(e >> 16);
+                    const uint32_t mask = (bt == b) ? 0x00FF00FFu : 0x00010001u * ((0xFF00u >> bt) & 0xFFu);
+#pragma unroll
+                    for (int r = 0; r < 8; ++r) {
+                        const uint32_t h01 = H[2 * r] & mask, h23 = H[2 * r + 1] & mask;
+                        fhfma_lo(acc[t][4 * r + 0], h01, xh);
+                        fhfma_hi(acc[t][4 * r + 1], h01, xh);
+                        fhfma_lo(acc[t][4 * r + 2], h23, xh);
+                        fhfma_hi(acc[t][4 * r + 3], h23, xh);
                     }
                 }
             }
