@@ -88,6 +88,7 @@ assign_kernel(const uint16_t* __restrict__ x, AssignParams p, uint8_t* __restric
     uint16_t* xs = reinterpret_cast<uint16_t*>(cnt + CNT_BYTES);    // raw fp16 patterns, local groups, current token
     uint8_t* glist = cnt + CNT_BYTES + (size_t)gpc * GQ_G * 2;      // local groups' lists
     __shared__ __align__(16) uint8_t gcs[MAXG][GQ_GCNT];
+    __shared__ __align__(16) uint8_t ubits[32 * GQ_G];              // union of the token widths, local groups (<= 32)
     __shared__ uint16_t tab[MAXG][10];                              // replicated: per-width counts of every group
     __shared__ uint16_t ltab[MAXG][8];                              // local groups: equal-key counts per cut
     __shared__ int s_rowL[NLEVEL][8 * NDIG];                        // this CTA's row sums, one array per level
@@ -268,7 +269,7 @@ assign_kernel(const uint16_t* __restrict__ x, AssignParams p, uint8_t* __restric
             }
             const uint32_t packed = (uint32_t)b[0] | ((uint32_t)b[1] << 8) | ((uint32_t)b[2] << 16) | ((uint32_t)b[3] << 24);
             *reinterpret_cast<uint32_t*>(bits + (size_t)t * K + g * GQ_G + 4 * lane) = packed;
-            uint32_t* u = reinterpret_cast<uint32_t*>(bits_union + g * GQ_G + 4 * lane);  // same thread every token
+            uint32_t* u = reinterpret_cast<uint32_t*>(ubits + lg * GQ_G + 4 * lane);  // union over tokens, shared memory
             if (t == 0) *u = packed;
             else *u = __vmaxu4(*u, packed);
         }
@@ -279,7 +280,8 @@ assign_kernel(const uint16_t* __restrict__ x, AssignParams p, uint8_t* __restric
     for (int lg = warp; lg < nloc; lg += AWARPS) {
         const int g = gl0 + lg;
         const int go = g * GQ_G + 4 * lane, lo = lg * GQ_G + 4 * lane;
-        const uint32_t bu4 = *reinterpret_cast<const uint32_t*>(bits_union + go);
+        const uint32_t bu4 = *reinterpret_cast<const uint32_t*>(ubits + lo);
+        *reinterpret_cast<uint32_t*>(bits_union + go) = bu4;
         uint32_t bt4[GRINQH_MAX_T];
         uint2 xv[GRINQH_MAX_T];
 #pragma unroll
