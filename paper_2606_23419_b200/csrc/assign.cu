@@ -277,11 +277,11 @@ assign_kernel(const uint16_t* __restrict__ x, AssignParams p, uint8_t* __restric
     }
 
     // ---- per-group lists of the local groups
+    const bool single_pass = nloc <= AWARPS;  // every warp has at most one group
     for (int lg = warp; lg < nloc; lg += AWARPS) {
         const int g = gl0 + lg;
         const int go = g * GQ_G + 4 * lane, lo = lg * GQ_G + 4 * lane;
         const uint32_t bu4 = *reinterpret_cast<const uint32_t*>(ubits + lo);
-        *reinterpret_cast<uint32_t*>(bits_union + go) = bu4;
         uint32_t bt4[GRINQH_MAX_T];
         uint2 xv[GRINQH_MAX_T];
 #pragma unroll
@@ -302,17 +302,19 @@ assign_kernel(const uint16_t* __restrict__ x, AssignParams p, uint8_t* __restric
                 myge = ge[c];
                 myn = ge[c] - ge[c + 1];
             }
-        if (lane < GQ_GCNT) {
-            const uint8_t v = (uint8_t)(lane <= 8 ? myge : 0);
-            gcnt_ge[g * GQ_GCNT + lane] = v;
-            gcs[lg][lane] = v;
-        }
+        const uint8_t gv = (uint8_t)(lane <= 8 ? myge : 0);
+        if (lane < GQ_GCNT) gcs[lg][lane] = gv;
         {   // every CTA gets the group's 9 per-width counts: lane = 9 * r' + c stores column c to CTA r' (and r' + 3, r' + 6)
             const int c = lane % 9, r0 = lane / 9;
             const int n = __shfl_sync(0xffffffffu, myn, c);
             if (lane < 27)
                 for (int r = r0; r < NC; r += 3) cluster.map_shared_rank(&tab[0][0], r)[g * 10 + c] = (uint16_t)n;
         }
+        // the cluster barrier only has to cover the counts just sent: arrive now (when this warp has no further group),
+        // then write the outputs to global memory in its shadow
+        if (single_pass) asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
+        *reinterpret_cast<uint32_t*>(bits_union + go) = bu4;
+        if (lane < GQ_GCNT) gcnt_ge[g * GQ_GCNT + lane] = gv;
 #pragma unroll
         for (int i = 0; i < 4; ++i) glist[lg * GQ_G + pos[i]] = (uint8_t)(4 * lane + i);
 #pragma unroll
@@ -328,7 +330,8 @@ assign_kernel(const uint16_t* __restrict__ x, AssignParams p, uint8_t* __restric
         __syncwarp();
         *reinterpret_cast<uint32_t*>(grows + go) = *reinterpret_cast<const uint32_t*>(glist + lo);
     }
-    cluster.sync();  // the last remote access of the kernel is before this barrier
+    if (!single_pass || warp >= nloc) asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
+    asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");  // the last remote access is before this barrier
     // ---- where each group's run of every width starts in the global list (every CTA scans its own copy)
     if (warp < 9) scan_groups(tab, warp, groups, lane, &s_tot[warp]);
     __syncthreads();
