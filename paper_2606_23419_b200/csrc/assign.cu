@@ -109,12 +109,8 @@ assign_kernel(const uint16_t* __restrict__ x, AssignParams p, uint8_t* __restric
     };
 
     pdl_launch_dependents();
-    pdl_wait();  // x may come from the previous kernel; the outputs may still be read by it
 
     for (int t = 0; t < p.T; ++t) {
-        // ---- load the token's local groups (raw patterns; the key is pattern & 0x7FFF)
-        for (int i = tid; i < nloc * (GQ_G / 4); i += AT)
-            reinterpret_cast<uint2*>(xs)[i] = reinterpret_cast<const uint2*>(x + (size_t)t * K + gl0 * GQ_G)[i];
         zero_region(0);
         if (tid < 8) {
             s_pre[0][tid] = (tid < nd) ? 0 : -1 - tid;  // level 0: one empty prefix shared by every cut
@@ -122,6 +118,11 @@ assign_kernel(const uint16_t* __restrict__ x, AssignParams p, uint8_t* __restric
             s_h[tid] = 0;
             s_tiebase[tid] = 0;
         }
+        // x may come from the previous kernel, and the outputs may still be read by it: nothing global before this
+        if (t == 0) pdl_wait();
+        // ---- load the token's local groups (raw patterns; the key is pattern & 0x7FFF)
+        for (int i = tid; i < nloc * (GQ_G / 4); i += AT)
+            reinterpret_cast<uint2*>(xs)[i] = reinterpret_cast<const uint2*>(x + (size_t)t * K + gl0 * GQ_G)[i];
         __syncthreads();
 
         if (p.use_thr) {  // the paper's run-time form: static thresholds, nothing to select
