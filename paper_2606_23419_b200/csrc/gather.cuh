@@ -5,7 +5,8 @@
 // the three butterfly stages of an 8x8 bit-matrix transpose on all four byte lanes at once and returns
 // V[r], r = 0..7, with   byte L of V[r] = truncated code (top B bits, low bits 0) of column 8 L + r.
 // Planes j >= B are treated as zero, so stages that would only move zeros fold away at compile time:
-// 48 logic/shift ops for B = 8, 28 for B = 4, about 20 for B = 2 (per 32 weights).
+// 36 + 12, 20 + 8 and 15 + 7 ops for B = 8, 4, 2 per 32 weights (logic or right shift on the half-rate pipe + left
+// shifts that the compiler issues as IMAD.SHL on the FMA pipe).
 //
 // Plain C++ on uint32_t so that the same code is unit-tested on the host (tests/test_host_logic.py).
 #pragma once
@@ -21,11 +22,26 @@ namespace gq {
 
 // transpose step on the pair (lo, hi) = (row i, row i+s) of every 8x8 byte-lane block:
 //   lo' = (lo & m) | ((hi & m) << s),   hi' = ((lo >> s) & m) | (hi & ~m),   m = low s bits of each 2s.
-template <int S>
+//   LOZ: lo is known to be zero (its planes are not fetched), so the step is a shift and two masks.
+template <int S, bool LOZ>
 GQ_HD void tstep(uint32_t& lo, uint32_t& hi) {
     constexpr uint32_t m = (S == 1) ? 0x55555555u : (S == 2) ? 0x33333333u : 0x0F0F0F0Fu;
-    const uint32_t nlo = (lo & m) | ((hi & m) << S);
-    const uint32_t nhi = ((lo >> S) & m) | (hi & ~m);
+    if (LOZ) {
+        lo = (hi << S) & ~m;
+        hi = hi & ~m;
+        return;
+    }
+    // two bit-selects under the one mask m (m << S == ~m): one LOP3 each after its shift.  The compiler rewrites the
+    // C form into and + or-and (2 LOP3 per output on the half-rate pipe), so the device path spells the LOP3 out.
+    const uint32_t H = hi << S, L = lo >> S;
+#if defined(__CUDA_ARCH__)
+    uint32_t nlo, nhi;
+    asm("lop3.b32 %0, %1, %2, %3, 0xE4;" : "=r"(nlo) : "r"(lo), "r"(H), "r"(m));  // (lo & m) | (H & ~m)
+    asm("lop3.b32 %0, %1, %2, %3, 0xE4;" : "=r"(nhi) : "r"(L), "r"(hi), "r"(m));  // (L & m) | (hi & ~m)
+#else
+    const uint32_t nlo = (lo & m) | (H & ~m);
+    const uint32_t nhi = (L & m) | (hi & ~m);
+#endif
     lo = nlo;
     hi = nhi;
 }
@@ -37,22 +53,22 @@ GQ_HD void gather(const uint32_t (&W)[8], uint32_t (&V)[8]) {
     // a[i] carries code bit i = plane 7 - i
 #pragma unroll
     for (int i = 0; i < 8; ++i) V[i] = (7 - i < B) ? W[7 - i] : 0u;
-    tstep<1>(V[6], V[7]);
-    if (B > 2) tstep<1>(V[4], V[5]);
+    tstep<1, false>(V[6], V[7]);
+    if (B > 2) tstep<1, false>(V[4], V[5]);
     if (B > 4) {
-        tstep<1>(V[0], V[1]);
-        tstep<1>(V[2], V[3]);
+        tstep<1, false>(V[0], V[1]);
+        tstep<1, false>(V[2], V[3]);
     }
-    tstep<2>(V[4], V[6]);
-    tstep<2>(V[5], V[7]);
+    tstep<2, (B <= 2)>(V[4], V[6]);
+    tstep<2, (B <= 2)>(V[5], V[7]);
     if (B > 4) {
-        tstep<2>(V[0], V[2]);
-        tstep<2>(V[1], V[3]);
+        tstep<2, false>(V[0], V[2]);
+        tstep<2, false>(V[1], V[3]);
     }
-    tstep<4>(V[0], V[4]);
-    tstep<4>(V[1], V[5]);
-    tstep<4>(V[2], V[6]);
-    tstep<4>(V[3], V[7]);
+    tstep<4, (B <= 4)>(V[0], V[4]);
+    tstep<4, (B <= 4)>(V[1], V[5]);
+    tstep<4, (B <= 4)>(V[2], V[6]);
+    tstep<4, (B <= 4)>(V[3], V[7]);
 }
 
 }  // namespace gq
