@@ -39,6 +39,24 @@ __global__ void k(uint32_t* out, uint32_t seed, long long* cyc) {
             if (MODE == 10) { // IMAD
                 asm volatile("mad.lo.u32 %0, %0, %1, %0;" : "+r"(a[i]) : "r"(a[(i + 1) & 7]));
             }
+            if (MODE == 11) asm volatile("mul.hi.u32 %0, %0, %1;" : "+r"(a[i]) : "r"(a[(i + 1) & 7]));
+            if (MODE == 12) { // IMAD.WIDE: 64-bit product + 64-bit addend
+                asm volatile("{.reg .b64 d; mov.b64 d, {%0,%1}; mad.wide.u32 d, %0, %2, d; mov.b64 {%0,%1}, d;}" : "+r"(a[i]), "+r"(a[(i + 4) & 7]) : "r"(seed));
+            }
+            if (MODE == 13) asm volatile("shr.u32 %0, %0, 1;" : "+r"(a[i]));
+            if (MODE == 14) asm volatile("add.u32 %0, %0, %1;" : "+r"(a[i]) : "r"(a[(i + 1) & 7]));
+            if (MODE == 15) { // 2 LOP3 + 1 mul.hi + 1 IMAD (a transpose pair with the right shift on the fma pipe)
+                asm volatile("lop3.b32 %0, %0, %1, %2, 0x96;" : "+r"(a[i]) : "r"(a[(i + 1) & 7]), "r"(seed));
+                asm volatile("lop3.b32 %0, %0, %1, %2, 0xE4;" : "+r"(a[(i+2)&7]) : "r"(a[(i + 3) & 7]), "r"(seed));
+                asm volatile("mul.hi.u32 %0, %0, %1;" : "+r"(a[(i+4)&7]) : "r"(seed));
+                asm volatile("mad.lo.u32 %0, %0, %1, %0;" : "+r"(a[(i+5)&7]) : "r"(seed));
+            }
+            if (MODE == 16) { // 2 LOP3 + 1 SHF + 1 IMAD (the pair as committed)
+                asm volatile("lop3.b32 %0, %0, %1, %2, 0x96;" : "+r"(a[i]) : "r"(a[(i + 1) & 7]), "r"(seed));
+                asm volatile("lop3.b32 %0, %0, %1, %2, 0xE4;" : "+r"(a[(i+2)&7]) : "r"(a[(i + 3) & 7]), "r"(seed));
+                asm volatile("shf.l.wrap.b32 %0, %0, %1, 3;" : "+r"(a[(i+4)&7]) : "r"(a[(i + 1) & 7]));
+                asm volatile("mad.lo.u32 %0, %0, %1, %0;" : "+r"(a[(i+5)&7]) : "r"(seed));
+            }
         }
     }
     long long t1 = clock64();
@@ -60,7 +78,7 @@ template <int MODE> void run(const char* name, int per_iter) {
 int main() {
     run<0>("FFMA 3reg", 1); run<1>("FHFMA (f32+=f16*f16)", 1); run<2>("LOP3", 1); run<3>("PRMT", 1); run<4>("SHF", 1);
     run<5>("FFMA2 (counts as 1 inst)", 1); run<6>("LOP3+FHFMA", 2); run<7>("PRMT+2FHFMA", 3); run<8>("FFMA reg*const", 1);
-    run<9>("HFMA2", 1); run<10>("IMAD", 1);
+    run<9>("HFMA2", 1); run<10>("IMAD", 1); run<11>("IMAD.HI", 1); run<12>("IMAD.WIDE", 1); run<13>("SHR", 1); run<14>("IADD", 1); run<15>("2LOP3+HI+IMAD", 4); run<16>("2LOP3+SHF+IMAD", 4);
     cudaError_t e = cudaGetLastError(); printf("err %s\n", cudaGetErrorString(e));
     return 0;
 }
