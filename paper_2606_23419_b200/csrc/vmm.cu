@@ -449,7 +449,7 @@ vmm_main_kernel(int K, int N, int Q, uint32_t rq, int ipw, int Sx, const uint32_
                     for (int r = 0; r < 8; ++r) {
                         float* dst = yacc + t * YSLOT + (8 * L + r) * 33 + lane;
                         float v = first ? 0.f : *dst;
-                        if (n_rows > 0) v += fmaf(sf[r], fmaf(acc[t][4 * r + L], CODE_SCALE, Phi[t]), zf[r] * X[t]);
+                        if (n_rows > 0) v = fmaf(zf[r], X[t], fmaf(sf[r], fmaf(acc[t][4 * r + L], CODE_SCALE, Phi[t]), v));
                         *dst = v;
                     }
             }
