@@ -492,22 +492,37 @@ vmm_main_kernel(int K, int N, int Q, uint32_t rq, int ipw, int Sx, const uint32_
         }
         __syncthreads();
         if (s_last) {
-            const int n = tile * TILE_COLS + 4 * tid;  // 4 columns per thread (the first 256 threads)
-            if (4 * tid < TILE_COLS && n < N) {
+            // every thread takes TILE_COLS / threads columns (4 with 8 warps, 2 with 16): the same bytes spread over
+            // all the CTA's threads, so one batch holds 16 or 32 partials per column in flight
+            constexpr int CPT = TILE_COLS / (VWT * 32);
+            constexpr int BATCH = (CPT == 2) ? 32 : 16;
+            using Vec = typename std::conditional<CPT == 2, float2, float4>::type;
+            const int n = tile * TILE_COLS + CPT * tid;
+            if (n < N) {
 #pragma unroll
                 for (int t = 0; t < T; ++t) {
-                    float4 a = make_float4(0.f, 0.f, 0.f, 0.f);
-                    for (int s0 = 0; s0 < Sx; s0 += 16) {  // 16 loads in flight, added in the fixed order
-                        float4 v[16];
+                    float a[CPT];
 #pragma unroll
-                        for (int j = 0; j < 16; ++j)
+                    for (int c = 0; c < CPT; ++c) a[c] = 0.f;
+                    for (int s0 = 0; s0 < Sx; s0 += BATCH) {  // BATCH loads in flight, added in the fixed order
+                        Vec v[BATCH];
+#pragma unroll
+                        for (int j = 0; j < BATCH; ++j)
                             if (s0 + j < Sx)
-                                v[j] = __ldcg(reinterpret_cast<const float4*>(part + ((size_t)(s0 + j) * T + t) * N + n));
+                                v[j] = __ldcg(reinterpret_cast<const Vec*>(part + ((size_t)(s0 + j) * T + t) * N + n));
 #pragma unroll
-                        for (int j = 0; j < 16; ++j)
-                            if (s0 + j < Sx) { a.x += v[j].x; a.y += v[j].y; a.z += v[j].z; a.w += v[j].w; }
+                        for (int j = 0; j < BATCH; ++j)
+                            if (s0 + j < Sx) {
+                                const float* f = reinterpret_cast<const float*>(&v[j]);
+#pragma unroll
+                                for (int c = 0; c < CPT; ++c) a[c] += f[c];
+                            }
                     }
-                    *reinterpret_cast<float4*>(y + (size_t)t * N + n) = a;
+                    Vec o;
+                    float* fo = reinterpret_cast<float*>(&o);
+#pragma unroll
+                    for (int c = 0; c < CPT; ++c) fo[c] = a[c];
+                    *reinterpret_cast<Vec*>(y + (size_t)t * N + n) = o;
                 }
             }
             if (tid == 0) tickets[tile] = 0;  // ready for the next launch on this workspace
