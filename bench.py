@@ -283,6 +283,10 @@ def run_native(args):
         for name, K, N, inp in fused:
             gq.grinqh_vmm_thresholds(x_dev[l][inp], thetas[inp], packed[l][name], y_dev[l][name], ws)
 
+    def step_rank_fused(l):      # the rank assignment made inside the VMM launch: 4 launches per step
+        for name, K, N, inp in fused:
+            gq.grinqh_vmm_rank(x_dev[l][inp], counts[K], packed[l][name], y_dev[l][name], ws)
+
     def step_main_only(l):       # the dominant kernel alone: the 4 VMM launches (assignments already on the device)
         for name, K, N, inp in fused:
             gq.grinqh_vmm(packed[l][name], assigns[l][inp], y_dev[l][name], ws)
@@ -362,6 +366,12 @@ def run_native(args):
         for i in range(3):
             g_thrf[i % L].replay()
         ms_thrf = timed(g_thrf, args.steps)
+        step_rank_fused(0)
+        stream.synchronize()
+        g_rf = capture(step_rank_fused)
+        for i in range(3):
+            g_rf[i % L].replay()
+        ms_rf = timed(g_rf, args.steps)
         thr_bits = float(np.mean([assigns[0][n].bits.float().mean().item() for n in in_dims]))
         for l in range(L):       # leave the rank-form assignments in the buffers (byte accounting below)
             for n, K in in_dims.items():
@@ -429,6 +439,8 @@ def run_native(args):
     line["threshold_assignment_fused"] = {"value": max_over_ranks([ms_thrf], dev)[0] * 1e3 / args.steps, "unit": UNIT,
                                           "what": "the same with the threshold assignment made inside the VMM launch "
                                                   "(grinqh_vmm_thresholds): 4 launches per step"}
+    line["rank_assignment_fused"] = {"value": max_over_ranks([ms_rf], dev)[0] * 1e3 / args.steps, "unit": UNIT,
+                                     "what": "the rank assignment made inside the VMM launch (grinqh_vmm_rank): 4 launches per step"}
     if ms_split:
         line["per_projection"] = {"value": ms_split * 1e3 / args.steps, "unit": UNIT,
                                   "what": "same step with one VMM launch per projection (4 assigns + 7 VMMs)"}

@@ -186,6 +186,19 @@ int grinqh_vmm_thresholds(const void* x_f16, int T, int K, int N, int group, con
                           float* y, void* workspace, size_t workspace_bytes, void* stream);
 
 /*
+ * grinqh_vmm_rank — the rank assignment of grinqh_assign (PAPER.md:271 top-p partition of the live vector,
+ * :61-65; ties to the lower index) made inside the VMM launch.  Every CTA selects the cut keys of x
+ * itself (a 5+5+5-bit radix select in shared memory), resolves ties in index order, and builds the lists of the
+ * groups it walks; no assignment kernel runs and no schedule is written.  y is bit-identical to grinqh_assign
+ * followed by grinqh_vmm.
+ *   x_f16   dev  [T, K] fp16        counts HOST [9], sum = K (GRINQH_ERR_MIX otherwise), read during the call
+ *   other arguments as in grinqh_vmm.
+ */
+int grinqh_vmm_rank(const void* x_f16, int T, int K, int N, int group, const uint32_t counts[9],
+                    const uint32_t* planes, const void* scales_f16, const void* zeros_f16,
+                    float* y, void* workspace, size_t workspace_bytes, void* stream);
+
+/*
  * Host-buffer decode call (the end-to-end entry): x comes from HOST memory, grinqh_assign + grinqh_vmm run, y ends
  * in HOST memory, all enqueued on `stream`.  With pinned (page-locked) buffers the kernels access host memory
  * directly (x is read once by the assignment, y is written by the VMM's second pass): no copy nodes.  With pageable

@@ -52,6 +52,8 @@ _lib.grinqh_vmm.restype = _i
 _lib.grinqh_vmm.argtypes = _VMM_COMMON + [_vp, _vp, _sz, _vp]
 _lib.grinqh_vmm_thresholds.restype = _i
 _lib.grinqh_vmm_thresholds.argtypes = [_vp, _i, _i, _i, _i, _vp, _vp, _vp, _vp, _vp, _vp, _sz, _vp]
+_lib.grinqh_vmm_rank.restype = _i
+_lib.grinqh_vmm_rank.argtypes = [_vp, _i, _i, _i, _i, _vp, _vp, _vp, _vp, _vp, _vp, _sz, _vp]
 _lib.grinqh_vmm_main.restype = _i
 _lib.grinqh_vmm_main.argtypes = _VMM_COMMON + [_vp, _sz, _vp]
 _lib.grinqh_vmm_reduce.restype = _i
@@ -63,7 +65,7 @@ _lib.grinqh_decode_host.argtypes = [_vp, _i, _i, _i, _i, _vp, _vp, _vp, _vp, _vp
 EXPORTS = ("grinqh_status_string", "grinqh_version", "grinqh_mix_to_counts", "grinqh_pack", "grinqh_unpack",
            "grinqh_assign_workspace_bytes", "grinqh_assign", "grinqh_assign_thresholds",
            "grinqh_calibrate_thresholds", "grinqh_vmm_workspace_bytes",
-           "grinqh_vmm_workspace_init", "grinqh_vmm", "grinqh_vmm_thresholds",
+           "grinqh_vmm_workspace_init", "grinqh_vmm", "grinqh_vmm_thresholds", "grinqh_vmm_rank",
            "grinqh_vmm_main", "grinqh_vmm_reduce", "grinqh_decode_host")
 
 
@@ -230,6 +232,19 @@ def grinqh_vmm_thresholds(x: torch.Tensor, theta, w: Packed, y: torch.Tensor | N
     _check(_lib.grinqh_vmm_thresholds(_dev(x, torch.float16, "x"), T, K, w.N, GROUP, th, w.planes.data_ptr(),
                                       w.scales.data_ptr(), w.zeros.data_ptr(), _dev(y, torch.float32, "y"),
                                       workspace.data_ptr(), nbytes, _stream(stream)), "grinqh_vmm_thresholds")
+    return y
+
+
+def grinqh_vmm_rank(x: torch.Tensor, counts, w: Packed, y: torch.Tensor | None = None,
+                    workspace: torch.Tensor | None = None, stream=None) -> torch.Tensor:
+    """y [T, N] = x . W with the rank assignment made inside the VMM launch (no assignment kernel)."""
+    T, K = x.shape
+    if y is None:
+        y = torch.empty((T, w.N), dtype=torch.float32, device=x.device)
+    workspace, nbytes = _ws(T, K, w.N, workspace, x.device)
+    _check(_lib.grinqh_vmm_rank(_dev(x, torch.float16, "x"), T, K, w.N, GROUP, _counts(counts), w.planes.data_ptr(),
+                                w.scales.data_ptr(), w.zeros.data_ptr(), _dev(y, torch.float32, "y"),
+                                workspace.data_ptr(), nbytes, _stream(stream)), "grinqh_vmm_rank")
     return y
 
 
