@@ -54,9 +54,21 @@ static inline VmmPlan vmm_plan(int T, int K, int N) {
     return pl;
 }
 
+// Measurement switch: GRINQH_BULK=1 selects the cp.async.bulk (TMA, SASS UBLKCP) + mbarrier form of the row copies.
+// It is correct and twice as slow as the cp.async (LDGSTS) form on B200 — a 128-byte bulk copy costs the TMA unit
+// ~24 cycles per SM (profiles/r02_bulk_ab.md) — so the default is LDGSTS.
+static bool use_bulk() {
+    static int v = -1;
+    if (v < 0) {
+        const char* f = getenv("GRINQH_BULK");
+        v = (f && atoi(f) == 1) ? 1 : 0;
+    }
+    return v != 0;
+}
+
 template <int VW, int MODE>
 static int launch_a16(const VmmArgs& a, const VmmPlan& pl) {
-    return launch_impl<1, VW, true, MODE>(a, pl);
+    return use_bulk() ? launch_impl<1, VW, true, MODE, true>(a, pl) : launch_impl<1, VW, true, MODE, false>(a, pl);
 }
 
 template <int MODE>

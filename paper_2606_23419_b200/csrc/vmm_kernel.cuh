@@ -47,7 +47,6 @@ constexpr int SLOT_BYTES = 1024;   // 8 planes x 128 B
 constexpr int YSLOT = 32 * 33;     // one warp's 1024 sums, padded: column 32*l + c lives at c*33 + l
 constexpr int GLC = 8;             // group lists a CTA builds once for all its warps (one token, in-kernel assignment)
 constexpr int MAXG = GQ_MAX_K / GQ_G;
-constexpr int ROW_COST = 12;       // cost of a row of width b = ROW_COST + b (loop bodies: ~94 / 106 / 137 instructions)
 constexpr uint32_t ENTRY_SZ = 0x80u;  // list entry is a scale/zero chunk (bits 0..1 = chunk); rows use bits 0..6
 constexpr size_t TICKET_BYTES = 16384;  // head of the workspace: one int per column tile, zero between launches
 
@@ -65,12 +64,12 @@ struct Cfg {
     static constexpr int YACC_OFF = RING * SLOT_BYTES;
     static constexpr int LIST_OFF = YACC_OFF + T * YSLOT * 4;
     static constexpr int XPHI_OFF = LIST_OFF + LISTN * 8 + (T - 1) * LISTN * 4;
-    static constexpr int WARP_BYTES = XPHI_OFF + 16 * T * 8;
+    static constexpr int MBAR_OFF = XPHI_OFF + 16 * T * 8;  // RING mbarriers (bulk-copy form)
+    static constexpr int WARP_BYTES = MBAR_OFF + RING * 8;
     // the assignment prologue aliases the warp regions: one token's keys and the select's 64-KB histogram
     static constexpr int KEYS_OFF = 0;
     static constexpr int HIST_OFF = GQ_MAX_K * 2;
-    static constexpr int GTEQ_OFF = HIST_OFF + 65536;  // keys above / equal to each cut per group: 2 x [MAXG][8] bytes
-    static constexpr int BASE_BYTES = cmax(VW * WARP_BYTES, GTEQ_OFF + 2 * MAXG * 8);  // the tie offsets live behind
+    static constexpr int BASE_BYTES = cmax(VW * WARP_BYTES, HIST_OFF + 65536);  // the tie offsets live behind
     static_assert(WARP_BYTES % 16 == 0, "warp regions stay 16-byte aligned");
     static_assert(T == 1 || VW == 8, "several tokens: 8 warps (registers: acc[T][32])");
 };
@@ -109,6 +108,27 @@ __device__ __forceinline__ void cp_async_wait() {
     asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory");
 }
 
+// TMA bulk copies (cp.async.bulk, SASS UBLKCP) completing on an mbarrier in shared memory
+__device__ __forceinline__ void mbar_init(uint32_t mbar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(mbar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t mbar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(mbar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t mbar, uint32_t parity) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "GQ_WAIT:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+        "@p bra GQ_DONE;\n\t"
+        "bra GQ_WAIT;\n\t"
+        "GQ_DONE:\n\t}" ::"r"(mbar), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t mbar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
+                 "l"(src), "r"(bytes), "r"(mbar) : "memory");
+}
+
 __device__ __forceinline__ void accumulate_row(const uint32_t (&V)[8], uint16_t xh, float* acc) {
 #pragma unroll
     for (int r = 0; r < 8; ++r) {
@@ -121,41 +141,13 @@ __device__ __forceinline__ void accumulate_row(const uint32_t (&V)[8], uint16_t 
     }
 }
 
-// cost of a group from its per-width counts ge[w] = rows of width >= w (bytes of cv):
-// sum_w n_w (ROW_COST + w) = ROW_COST ge[1] + sum_{w>=1} ge[w]
-__device__ __forceinline__ int group_cost(const uint4 cv) {
-    const uint32_t s = __dp4a(cv.x & 0xFFFFFF00u, 0x01010101u, 0u) + __dp4a(cv.y, 0x01010101u, 0u) + (cv.z & 0xFFu);
-    return (int)(ROW_COST * ((cv.x >> 8) & 0xFFu) + s);
-}
-
-// First list position of a group whose start cost is >= off (rows in width desc order), lane-parallel: lane w = 1..8
-// looks at the rows of width w.  gc = the group's 16 count bytes in shared memory.  Same result on every lane.
-__device__ __forceinline__ int pos_from_cost(const uint8_t* gc, int off, int lane) {
-    const int w = (lane >= 1 && lane <= 8) ? lane : 0;
-    const int hi = w ? (int)gc[w + 1] : 0;                 // rows of larger width = position of the class
-    const int n = w ? (int)gc[w] - hi : 0;
-    const int c = ROW_COST + w;
-    int cum = n * c;                                       // suffix sum over larger widths: lanes above
-#pragma unroll
-    for (int d = 1; d < 8; d <<= 1) {
-        const int o = __shfl_down_sync(0xffffffffu, cum, d);
-        if (lane + d <= 8) cum += o;
-    }
-    const int before = cum - n * c;                        // cost of all rows of larger width
-    const bool mine = w && off >= before && off < before + n * c;
-    const uint32_t bal = __ballot_sync(0xffffffffu, mine);
-    const int pos = hi + (off - before + c - 1) / c;
-    if (bal == 0) return (int)gc[1];                       // off at or beyond the group's cost
-    return __shfl_sync(0xffffffffu, pos, __ffs(bal) - 1);
-}
-
 // A16: every plane row is 16-byte aligned (N % 128 == 0) -> LDGSTS.128, 4 planes per instruction;
 // otherwise each lane copies its own word of every plane with 4-byte cp.async.
 //
 // gsched[t][g*128 + p] (MODE_SCHED, written by grinqh_assign) is position p of group g's list for token t:
 //   bits 0..7 local row r | 8..11 b_t (token's width) | 12..15 b (union width = planes fetched) | 16..31 x_t[r] fp16
 // The in-kernel forms build the same entries from xraw.
-template <int T, int VW, bool A16, int MODE>
+template <int T, int VW, bool A16, int MODE, bool BULK>
 __global__ void __launch_bounds__(VW * 32, 1)
 vmm_kernel(int K, int N, int Sx, int fused, const uint32_t* __restrict__ planes, const __half* __restrict__ scales,
            const __half* __restrict__ zeros, const uint32_t* __restrict__ gsched, const uint8_t* __restrict__ gcnt_ge,
@@ -164,12 +156,10 @@ vmm_kernel(int K, int N, int Sx, int fused, const uint32_t* __restrict__ planes,
     using C = Cfg<T, VW>;
     constexpr int RING = C::RING, NT = C::NT;
     extern __shared__ __align__(16) uint8_t smem[];
-    __shared__ __align__(16) uint8_t s_gcnt[MAXG][GQ_GCNT];  // per-group counts ge[0..9] of the union widths
-    __shared__ uint32_t s_glist[GLC][GQ_G];                 // lists of the first GLC groups of this CTA's range
-    __shared__ int s_pref[MAXG + 1];                         // exclusive prefix of the groups' costs
+    __shared__ uint32_t s_glist[GLC][GQ_G];  // lists of the first GLC groups of this CTA's range
     __shared__ __align__(16) TokenCuts s_tc[T];
     __shared__ SelectScratch s_sel;
-    __shared__ int s_wsum[32], s_total, s_last;
+    __shared__ int s_last;
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int tile = blockIdx.x, sx = blockIdx.y;
@@ -186,8 +176,6 @@ vmm_kernel(int K, int N, int Sx, int fused, const uint32_t* __restrict__ planes,
     float* yacc = reinterpret_cast<float*>(wbase + C::YACC_OFF);
     const uint32_t ring_s = (uint32_t)__cvta_generic_to_shared(wbase + C::RING_OFF);
     uint16_t* s_tie = reinterpret_cast<uint16_t*>(smem + C::BASE_BYTES);  // [T][groups][8] ordered tie offsets
-    uint8_t (*s_gt)[8] = reinterpret_cast<uint8_t (*)[8]>(smem + C::GTEQ_OFF);  // prologue only (aliases warp regions)
-    uint8_t (*s_eq)[8] = s_gt + MAXG;
 
 #ifdef GQ_TIMING
     long long stamp[16];
@@ -199,11 +187,9 @@ vmm_kernel(int K, int N, int Sx, int fused, const uint32_t* __restrict__ planes,
     GQ_STAMP();
     pdl_launch_dependents();
 
-    // ================================================================== prologue: per-group counts of the union widths
+    // ================================================================== prologue: the cuts and the ordered tie offsets
     if (MODE == MODE_SCHED) {
         pdl_wait();  // nothing global is touched before the previous kernel has finished
-        for (int g = tid; g < groups; g += NT)
-            *reinterpret_cast<uint4*>(s_gcnt[g]) = *reinterpret_cast<const uint4*>(gcnt_ge + (size_t)g * GQ_GCNT);
     } else {
         uint16_t* skeys = reinterpret_cast<uint16_t*>(smem + C::KEYS_OFF);
         if (MODE == MODE_RANK) {  // the select's histogram: cleared while the previous kernel is still running
@@ -220,8 +206,6 @@ vmm_kernel(int K, int N, int Sx, int fused, const uint32_t* __restrict__ planes,
                                 t + 1 < T, &s_sel, &s_tc[t]);
                 GQ_STAMP();
             } else {
-                for (int i = tid; i < (K >> 3); i += NT)
-                    reinterpret_cast<uint4*>(skeys)[i] = reinterpret_cast<const uint4*>(xraw + (size_t)t * K)[i];
                 if (tid < 8) {
                     s_tc[t].thr[tid] = cp.thr[tid];
                     s_tc[t].take[tid] = 0;
@@ -234,177 +218,95 @@ vmm_kernel(int K, int N, int Sx, int fused, const uint32_t* __restrict__ planes,
                 __syncthreads();
             }
             const uint32_t split = s_tc[t].split;
-            // ---- per group and cut: keys above and keys equal (one token: every group's per-width counts follow
-            //      from them; several tokens: only the ordered tie offsets are needed, and only if a cut splits)
-            if (T == 1 || split) {
+            if (split) {
+                // ---- a cut splits a run of equal keys: per group the number of keys equal to each such cut (thread =
+                //      8 consecutive keys, 16 threads = one group: a half-warp reduction), then their exclusive prefix
+                //      over the groups = the ordered tie offsets (ties go to the lower index)
                 uint16_t* tie = s_tie + (size_t)t * groups * 8;
 #pragma unroll 1
-                for (int g = warp; g < groups; g += VW) {
-                    const uint2 kv = *reinterpret_cast<const uint2*>(skeys + g * GQ_G + 4 * lane);
-                    int m[4];
-                    keys4(kv, m);
-                    uint32_t mine = 0;
-#pragma unroll 1
-                    for (int d = 0; d < nd; ++d) {
-                        const int th = s_tc[t].thr[d];
-                        uint32_t c2 = 0;  // keys above in the low half, keys equal in the high half
+                for (int c0 = warp * 32; c0 < (K >> 3); c0 += NT) {  // (warp-uniform bounds: every lane shuffles)
+                    const int c = c0 + lane;
+                    const bool valid = c < (K >> 3);
+                    const uint4 kv = valid ? reinterpret_cast<const uint4*>(skeys)[c] : make_uint4(~0u, ~0u, ~0u, ~0u);
+                    const uint32_t kw[4] = {kv.x, kv.y, kv.z, kv.w};
+                    uint32_t pk[2] = {0u, 0u};  // equal counts of cuts 0..3 and 4..7, 8 bits each (a group has 128 keys)
 #pragma unroll
-                        for (int i = 0; i < 4; ++i) c2 += (m[i] > th) ? 1u : ((m[i] == th) ? 0x10000u : 0u);
-                        c2 = __reduce_add_sync(0xffffffffu, c2);
-                        if (lane == d) mine = c2;
+                    for (int d = 0; d < 8; ++d) {
+                        if (d < nd) {  // uniform
+                            const uint32_t th = (uint32_t)s_tc[t].thr[d];
+                            uint32_t ce = 0;
+#pragma unroll
+                            for (int j = 0; j < 8; ++j) ce += (((kw[j >> 1] >> (16 * (j & 1))) & 0x7FFFu) == th) ? 1u : 0u;
+                            pk[d >> 2] += ce << (8 * (d & 3));
+                        }
                     }
-                    if (lane < 8) {
-                        s_gt[g][lane] = (uint8_t)(mine & 0xFFFFu);
-                        s_eq[g][lane] = (uint8_t)(mine >> 16);
+#pragma unroll
+                    for (int o = 8; o >= 1; o >>= 1) {  // the 16 lanes of a group
+                        pk[0] += __shfl_xor_sync(0xffffffffu, pk[0], o);
+                        if (nd > 4) pk[1] += __shfl_xor_sync(0xffffffffu, pk[1], o);
+                    }
+                    if (valid && (lane & 15) < 8) {
+                        const int d = lane & 15;
+                        tie[(c >> 4) * 8 + d] = (uint16_t)((pk[d >> 2] >> (8 * (d & 3))) & 0xFFu);
                     }
                 }
                 __syncthreads();
-                // ---- equal counts -> exclusive prefix over the groups (warp d scans cut d, 32 groups at a time)
 #pragma unroll 1
-                for (int d = warp; d < nd; d += VW) {
+                for (int d = warp; d < nd; d += VW) {  // (up to 8 rounds of 32 groups: independent scans, then the carries)
+                    int v[8], inc[8];
+#pragma unroll
+                    for (int r = 0; r < 8; ++r) {
+                        const int g = 32 * r + lane;
+                        v[r] = (g < groups) ? (int)tie[g * 8 + d] : 0;
+                        inc[r] = (32 * r < groups) ? warp_incl_scan_i(v[r], lane) : 0;
+                    }
                     int carry = 0;
-#pragma unroll 1
-                    for (int g0 = 0; g0 < groups; g0 += 32) {
-                        const int g = g0 + lane;
-                        const int v = (g < groups) ? (int)s_eq[g][d] : 0;
-                        const int incl = warp_incl_scan_i(v, lane);
-                        if (g < groups) tie[g * 8 + d] = (uint16_t)(carry + incl - v);
-                        carry += __shfl_sync(0xffffffffu, incl, 31);
+#pragma unroll
+                    for (int r = 0; r < 8; ++r) {
+                        const int g = 32 * r + lane;
+                        if (g < groups) tie[g * 8 + d] = (uint16_t)(carry + inc[r] - v[r]);
+                        carry += __shfl_sync(0xffffffffu, inc[r], 31);
                     }
                 }
                 __syncthreads();
             }
         }
-        GQ_STAMP();
-        if (T == 1) {
-            // ---- keys above cut d in group g = gt + (split ? clamp(take - tie offset, 0, eq) : eq), and a row has
-            //      >= w bits iff its key is above cut cw[w].  One thread per (group, width).
-            const uint32_t split = s_tc[0].split;
-#pragma unroll 1
-            for (int i = tid; i < groups * 8; i += NT) {
-                const int g = i >> 3, w = (i & 7) + 1, d = cp.cw[w];
-                int above = 0;
-                if (d >= 0) {
-                    const int eq = s_eq[g][d];
-                    above = s_gt[g][d];
-                    if ((split >> d) & 1u) above += max(0, min(s_tc[0].take[d] - (int)s_tie[g * 8 + d], eq));
-                    else above += eq;
-                }
-                s_gcnt[g][w] = (uint8_t)above;
-                if (w == 1) {
-                    s_gcnt[g][0] = GQ_G;
-                    s_gcnt[g][9] = 0;
-                }
-            }
-        } else {
-            // ---- several tokens: the union width of a key is the maximum over the tokens: per-key widths, one warp
-            //      per group
-#pragma unroll 1
-            for (int g = warp; g < groups; g += VW) {
-                int bu[4] = {0, 0, 0, 0};
-#pragma unroll 1
-                for (int t = 0; t < T; ++t) {
-                    int m[4], b[4];
-                    keys4(*reinterpret_cast<const uint2*>(xraw + (size_t)t * K + g * GQ_G + 4 * lane), m);
-                    widths4(m, &s_tc[t], cp.mult, nd, s_tie + ((size_t)t * groups + g) * 8, lane, b);
-#pragma unroll
-                    for (int i = 0; i < 4; ++i) bu[i] = max(bu[i], b[i]);
-                }
-                int pos[4], ge[10];
-                partition128(bu, lane, pos, ge);
-                int myge = 0;
-#pragma unroll
-                for (int c = 0; c <= 9; ++c)
-                    if (lane == c) myge = ge[c];
-                if (lane < GQ_GCNT) s_gcnt[g][lane] = (uint8_t)(lane <= 9 ? myge : 0);
-            }
-        }
     }
-    __syncthreads();
-    // ---- exclusive prefix of the groups' costs (block scan, NT groups at a time)
-    {
-        int carry = 0;
-#pragma unroll 1
-        for (int g0 = 0; g0 < groups; g0 += NT) {
-            const int g = g0 + tid;
-            const int c = (g < groups) ? group_cost(*reinterpret_cast<const uint4*>(s_gcnt[g])) : 0;
-            const int incl = warp_incl_scan_i(c, lane);
-            if (lane == 31) s_wsum[warp] = incl;
-            __syncthreads();
-            if (warp == 0) {
-                const int v = (lane < VW) ? s_wsum[lane] : 0;
-                const int i2 = warp_incl_scan_i(v, lane);
-                s_wsum[lane] = i2 - v;
-                if (lane == 31) s_total = i2;
-            }
-            __syncthreads();
-            if (g < groups) s_pref[g] = carry + s_wsum[warp] + incl - c;
-            carry += s_total;
-            if (g0 + NT < groups) __syncthreads();  // s_wsum is reused
-        }
-        if (tid == 0) s_pref[groups] = carry;
-    }
-    GQ_STAMP();
-    __syncthreads();
-    GQ_STAMP();
 
-    // ================================================================== the warp's range of the tile's row stream
-    int g_a, pos_a, g_b, pos_b;  // rows [(g_a, pos_a), (g_b, pos_b)) in stream order; g_b may be `groups`
-    int G0 = 0;                  // first group of the CTA's range
-    {
-        const int total = s_pref[groups];
-        const int S = Sx * VW, ws = sx * VW + warp;
-        // total <= 256 * 128 * 20 < 2^20 and S <= 2^12 when it matters: 32-bit products (64-bit division is ~100 instructions)
-        const bool small = total < (1 << 20) && S <= (1 << 12);
-        auto bound = [&](int i) {
-            return small ? (int)(((uint32_t)total * (uint32_t)i) / (uint32_t)S) : (int)(((long long)total * i) / S);
-        };
-        // the group holding cost c = the last g with pref[g] <= c (g = groups when c == total): 8-way blocks first
-        auto locate_group = [&](int c) {
-            const int gi = min(8 * lane, groups);
-            const uint32_t b1 = __ballot_sync(0xffffffffu, 8 * lane <= groups && s_pref[gi] <= c);
-            const int blk = 31 - __clz(b1);  // lane 0 always qualifies (pref[0] = 0 <= c)
-            const int gj = min(8 * blk + (lane & 7), groups);
-            const uint32_t b2 = __ballot_sync(0xffffffffu, lane < 8 && 8 * blk + lane <= groups && s_pref[gj] <= c);
-            return 8 * blk + (31 - __clz(b2));
-        };
-        const int lo = bound(ws), hi = bound(ws + 1);
-        g_a = locate_group(lo);
-        pos_a = (g_a < groups) ? pos_from_cost(s_gcnt[g_a], lo - s_pref[g_a], lane) : 0;
-        g_b = locate_group(hi);
-        pos_b = (g_b < groups) ? pos_from_cost(s_gcnt[g_b], hi - s_pref[g_b], lane) : 0;
-        if (T == 1 && MODE != MODE_SCHED) {
-            // ---- the lists of the first GLC groups of the CTA's range are made once, by one warp each, from the keys
-            //      still in shared memory (every warp of the CTA walks one or two of the same few groups)
-            const int cta_hi = bound((sx + 1) * VW);
-            G0 = locate_group(bound(sx * VW));
+    // ================================================================== the warp's range of the tile's slots
+    // Group g owns slots 128 g .. 128 g + 127; slot s holds position brev7(s) of the group's (width desc, index asc)
+    // list, so ANY run of consecutive slots sees the group's width mix (and its share of the b = 0 rows, which are
+    // skipped): warp slot ws of the tile's S = Sx * VW warps takes slots [ws K / S, (ws + 1) K / S) — balanced without
+    // knowing a single width, so nothing has to be counted or scanned before the first row can be fetched.
+    const int S = Sx * VW, ws = sx * VW + warp;
+    const int slot_lo = (int)(((uint32_t)K * (uint32_t)ws) / (uint32_t)S);        // K <= 2^15, S < 2^17
+    const int slot_hi = (int)(((uint32_t)K * (uint32_t)(ws + 1)) / (uint32_t)S);
+    const int G0 = (int)(((uint32_t)K * (uint32_t)(sx * VW)) / (uint32_t)S) >> 7;  // first group of the CTA's range
+    if (T == 1 && MODE != MODE_SCHED) {
+        // ---- the lists of the first GLC groups of the CTA's range are made once, by one warp each (every warp of the
+        //      CTA walks one or two of the same few groups)
+        const int cta_hi = (int)(((uint32_t)K * (uint32_t)((sx + 1) * VW)) / (uint32_t)S);
 #pragma unroll 1
-            for (int gi = warp; gi < GLC; gi += VW) {
-                const int g = G0 + gi;
-                if (g >= groups || s_pref[g] >= cta_hi) break;
-                const uint16_t* skeys = reinterpret_cast<const uint16_t*>(smem + C::KEYS_OFF);
-                const uint2 xv = *reinterpret_cast<const uint2*>(skeys + g * GQ_G + 4 * lane);
-                int m[4], b[4], pos[4], ge[10];
-                keys4(xv, m);
-                widths4(m, &s_tc[0], cp.mult, nd, s_tie + (size_t)g * 8, lane, b);
-                partition128(b, lane, pos, ge);
-                const uint32_t xs[4] = {xv.x & 0xFFFFu, xv.x >> 16, xv.y & 0xFFFFu, xv.y >> 16};
+        for (int gi = warp; gi < GLC; gi += VW) {
+            const int g = G0 + gi;
+            if (g >= groups || g * GQ_G >= cta_hi) break;
+            const uint2 xv = (MODE == MODE_RANK)
+                                 ? *reinterpret_cast<const uint2*>(reinterpret_cast<const uint16_t*>(smem + C::KEYS_OFF) +
+                                                                   g * GQ_G + 4 * lane)
+                                 : *reinterpret_cast<const uint2*>(xraw + g * GQ_G + 4 * lane);
+            int m[4], b[4], pos[4], ge[10];
+            keys4(xv, m);
+            widths4(m, &s_tc[0], cp.mult, nd, s_tie + (size_t)g * 8, lane, b);
+            partition128(b, lane, pos, ge);
+            const uint32_t xs[4] = {xv.x & 0xFFFFu, xv.x >> 16, xv.y & 0xFFFFu, xv.y >> 16};
 #pragma unroll
-                for (int i = 0; i < 4; ++i)
-                    s_glist[gi][pos[i]] = (uint32_t)(4 * lane + i) | ((uint32_t)b[i] << 8) | ((uint32_t)b[i] << 12) | (xs[i] << 16);
-            }
+            for (int i = 0; i < 4; ++i)
+                s_glist[gi][pos[i]] = (uint32_t)(4 * lane + i) | ((uint32_t)b[i] << 8) | ((uint32_t)b[i] << 12) | (xs[i] << 16);
         }
     }
     GQ_STAMP();
     __syncthreads();  // from here on the warp regions belong to their warps
     GQ_STAMP();
-
-    // the warp's accumulator tile starts at zero
-    {
-        float4* yz = reinterpret_cast<float4*>(yacc);
-#pragma unroll 1
-        for (int i = lane; i < T * YSLOT / 4; i += 32) yz[i] = make_float4(0.f, 0.f, 0.f, 0.f);
-    }
 
     // per-lane copy geometry: lane copies chunk `seg` (16 B) of plane pj (and pj + 4); pjx = 99 disables the lane
     const int pj = lane >> 3, seg = lane & 7;
@@ -414,94 +316,143 @@ vmm_kernel(int K, int N, int Sx, int fused, const uint32_t* __restrict__ planes,
                               (A16 ? (size_t)pj * pbytes + (size_t)(tile * 32 + seg * 4) * 4 : (size_t)word * 4);
     const uint32_t lane_dst = A16 ? ring_s + pj * 128 + seg * 16 : ring_s + lane * 4;
     const size_t hi_off = 4 * pbytes;  // planes 4..7 of the same row
+    // bulk-copy form: lane j copies the whole 128-byte segment of plane j with one cp.async.bulk; slot v mod RING has
+    // its own mbarrier (one arrival = the expect_tx of lane 0, then the bytes)
+    const uint32_t mbar_s = (uint32_t)__cvta_generic_to_shared(wbase + C::MBAR_OFF);
+    const uint32_t segbytes = (uint32_t)min(128, max(0, (int)rowbytes - tile * 128));
+    const uint8_t* bulk_src = reinterpret_cast<const uint8_t*>(planes) + (size_t)lane * pbytes + (size_t)tile * 128;
+    if (BULK) {
+        if (lane == 0) {
+#pragma unroll 1
+            for (int i = 0; i < RING; ++i) mbar_init(mbar_s + i * 8, 1);
+            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        }
+        __syncwarp();
+    }
 
     // ================================================================== list: pieces of group segments appended ahead of the copies
     // entry = {word, byte offset of the row inside a plane}; word of a row: the gsched format; word of a scale/zero
     // chunk: ENTRY_SZ | chunk L (bits 0..1) | group (bits 8..15) | X/Phi slot (bits 16..19).
     constexpr int LN = C::LISTN;
-    constexpr int SUBMAX = LN / 2 - 4;  // rows appended per call: the list holds a piece + what is still in flight
     uint2* list = reinterpret_cast<uint2*>(wbase + C::LIST_OFF);              // [LN]
     uint32_t* tok = reinterpret_cast<uint32_t*>(wbase + C::LIST_OFF + LN * 8);  // [T-1][LN] words of tokens 1..T-1
     float2* xphi = reinterpret_cast<float2*>(wbase + C::XPHI_OFF);            // [16][T] {X, Phi} of the segments in flight
     int app = 0;                  // list entries appended so far
     int iv = 0, cv = 0;           // next entry to issue / to consume
-    int seg_g = g_a, seg_p = pos_a, seg_p1 = 0, segj = 0;  // group being appended, next position, end position
+    int seg_s = slot_lo;          // next slot to append (a piece = the slots of one half of one group's positions)
+    int seg_half = 0, segj = 0;
+    bool seg_rows = false;        // the current segment has appended at least one row
+    uint32_t gw[T][4];            // the current group: words of the lane's 4 rows / positions, their positions,
+    int gpos[4], gnz = 0;         // whether they are in the warp's slots, rows with b > 0
+    bool gin[4];
     float Xrun[T], Prun[T];       // X = sum x, Phi = sum x phi_b over the segment's rows appended so far
 #pragma unroll
     for (int t = 0; t < T; ++t) Xrun[t] = Prun[t] = 0.f;
 
-    auto seg_end = [&](int g) { return (g == g_b) ? min(pos_b, (int)s_gcnt[g][1]) : (int)s_gcnt[g][1]; };
-    // skips groups without rows for this warp; false when the range is exhausted
-    auto more_rows = [&]() {
-        while (seg_g < groups && seg_g <= g_b) {
-            seg_p1 = seg_end(seg_g);
-            if (seg_p < seg_p1) return true;
-            ++seg_g;
-            seg_p = 0;
-        }
-        return false;
-    };
+    auto more_rows = [&]() { return seg_s < slot_hi; };
 
-    // appends up to SUBMAX rows of the current group (+ the 4 chunk entries when they were its last)
+    // appends the warp's rows of the current group whose positions lie in half `seg_half` (positions 64 h .. 64 h + 63),
+    // in position order (so width classes stay together), + the 4 chunk entries after the second half
     auto append_piece = [&]() {
-        const int g = seg_g, p0 = seg_p;
-        const int n = min(seg_p1 - p0, SUBMAX);
-        if (MODE == MODE_SCHED) {
-#pragma unroll 1
-            for (int i = lane; i < n; i += 32) {
-                list[(app + i) & (LN - 1)].x = gsched[(size_t)g * GQ_G + p0 + i];
+        const int g = seg_s >> 7;
+        const int a = seg_s & 127, b_ = min(slot_hi - g * GQ_G, GQ_G);  // the warp's slots of this group: [a, b_)
+        // lane l looks at positions 4 l .. 4 l + 3: brev7(4 l + i) = (brev2(i) << 5) | brev5(l)
+        const bool direct = MODE == MODE_SCHED || (T == 1 && g - G0 < GLC);  // the list exists: position = 4 lane + i
+        if (seg_half == 0) {  // the group's words are fetched / made once and kept for both halves
+            if (direct) {
+                const int rl = (int)(__brev((uint32_t)lane) >> 27);
+                const int sl[4] = {rl, 64 + rl, 32 + rl, 96 + rl};
+                // (rows with b = 0 sit at the end of the list and say so themselves: no count is needed)
+                gnz = GQ_G;
 #pragma unroll
-                for (int t = 1; t < T; ++t)
-                    tok[(t - 1) * LN + ((app + i) & (LN - 1))] = gsched[(size_t)t * K + g * GQ_G + p0 + i];
-            }
-        } else if (T == 1 && g - G0 < GLC) {
-#pragma unroll 1
-            for (int i = lane; i < n; i += 32) list[(app + i) & (LN - 1)].x = s_glist[g - G0][p0 + i];
-        } else {
-            uint2 xv[T];
-            int bt[T][4], bu[4] = {0, 0, 0, 0}, pos[4], ge[10];
+                for (int i = 0; i < 4; ++i) {
+                    gpos[i] = 4 * lane + i;
+                    bool in = sl[i] >= a && sl[i] < b_;
 #pragma unroll
-            for (int t = 0; t < T; ++t) {
-                xv[t] = *reinterpret_cast<const uint2*>(xraw + (size_t)t * K + g * GQ_G + 4 * lane);
-                int m[4];
-                keys4(xv[t], m);
-                widths4(m, &s_tc[t], cp.mult, nd, s_tie + ((size_t)t * groups + g) * 8, lane, bt[t]);
+                    for (int t = 0; t < T; ++t)
+                        gw[t][i] = !in ? 0u
+                                   : (MODE == MODE_SCHED) ? gsched[(size_t)t * K + g * GQ_G + gpos[i]]
+                                                          : s_glist[g - G0][gpos[i]];
+                    gin[i] = in && ((gw[0][i] >> 12) & 15u) != 0u;
+                }
+            } else {
+                uint2 xv[T];
+                int bt[T][4], bu[4], ge[10];
 #pragma unroll
-                for (int i = 0; i < 4; ++i) bu[i] = max(bu[i], bt[t][i]);
-            }
-            partition128(bu, lane, pos, ge);
+                for (int i = 0; i < 4; ++i) bu[i] = 0;
 #pragma unroll
-            for (int t = 0; t < T; ++t) {
-                const uint32_t xs[4] = {xv[t].x & 0xFFFFu, xv[t].x >> 16, xv[t].y & 0xFFFFu, xv[t].y >> 16};
+                for (int t = 0; t < T; ++t) {
+                    xv[t] = *reinterpret_cast<const uint2*>(xraw + (size_t)t * K + g * GQ_G + 4 * lane);
+                    int m[4];
+                    keys4(xv[t], m);
+                    widths4(m, &s_tc[t], cp.mult, nd, s_tie + ((size_t)t * groups + g) * 8, lane, bt[t]);
 #pragma unroll
-                for (int i = 0; i < 4; ++i)
-                    if (pos[i] >= p0 && pos[i] < p0 + n) {
-                        const uint32_t w = (uint32_t)(4 * lane + i) | ((uint32_t)bt[t][i] << 8) | ((uint32_t)bu[i] << 12) |
-                                           (xs[i] << 16);
-                        const int idx = (app + pos[i] - p0) & (LN - 1);
-                        if (t == 0) list[idx].x = w;
-                        else tok[(t - 1) * LN + idx] = w;
+                    for (int i = 0; i < 4; ++i) bu[i] = max(bu[i], bt[t][i]);
+                }
+                partition128(bu, lane, gpos, ge);
+                gnz = ge[1];
+#pragma unroll
+                for (int i = 0; i < 4; ++i) {
+                    const int s_ = (int)(__brev((uint32_t)gpos[i]) >> 25);
+                    gin[i] = s_ >= a && s_ < b_ && gpos[i] < gnz;
+#pragma unroll
+                    for (int t = 0; t < T; ++t) {
+                        const uint32_t xs = (i == 0) ? (xv[t].x & 0xFFFFu) : (i == 1) ? (xv[t].x >> 16)
+                                            : (i == 2) ? (xv[t].y & 0xFFFFu) : (xv[t].y >> 16);
+                        gw[t][i] = (uint32_t)(4 * lane + i) | ((uint32_t)bt[t][i] << 8) | ((uint32_t)bu[i] << 12) | (xs << 16);
                     }
+                }
             }
         }
-        __syncwarp();
-        // ---- common to all forms (same lane <-> position mapping, so every form sums X and Phi in the same order):
-        //      row byte offsets, and this piece's share of the segment's X and Phi
+        bool have[4];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) have[i] = gin[i] && (gpos[i] >> 6) == seg_half;
+        // ---- rank of every kept position among the kept positions of this half.  inc[i] = kept positions of the form
+        //      4 l' + i (bit l'), the same on every lane: position p = 4 q + r is preceded by those with l' < q, plus
+        //      l' = q for i < r.
+        uint32_t inc[4];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            bool k;  // is position 4 lane + i kept?
+            if (direct) {
+                k = have[i];
+            } else {
+                const int p = 4 * lane + i;
+                const int s_ = (int)(__brev((uint32_t)p) >> 25);
+                k = s_ >= a && s_ < b_ && p < gnz && (p >> 6) == seg_half;
+            }
+            inc[i] = __ballot_sync(0xffffffffu, k);
+        }
+        const int n = __popc(inc[0]) + __popc(inc[1]) + __popc(inc[2]) + __popc(inc[3]);
+        const uint32_t gbase = (uint32_t)g * GQ_G * rowbytes;
         float Xp[T], Pp[T];
 #pragma unroll
         for (int t = 0; t < T; ++t) Xp[t] = Pp[t] = 0.f;
-        const uint32_t gbase = (uint32_t)g * GQ_G * rowbytes;
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            if (have[i]) {
+                const int q = gpos[i] >> 2, r = gpos[i] & 3;
+                const uint32_t below = (1u << q) - 1u, upto = below | (1u << q);
+                const int rank = __popc(inc[0] & (r > 0 ? upto : below)) + __popc(inc[1] & (r > 1 ? upto : below)) +
+                                 __popc(inc[2] & (r > 2 ? upto : below)) + __popc(inc[3] & below);
+                const int idx = (app + rank) & (LN - 1);
+                list[idx] = make_uint2(gw[0][i], gbase + (gw[0][i] & 0x7Fu) * rowbytes);
+#pragma unroll
+                for (int t = 1; t < T; ++t) tok[(t - 1) * LN + idx] = gw[t][i];
+            }
+        }
+        __syncwarp();
+        // ---- this piece's share of the segment's X and Phi, summed in list order by every form (same bits)
 #pragma unroll 1
         for (int i = lane; i < n; i += 32) {
             const int idx = (app + i) & (LN - 1);
-            const uint32_t w0 = list[idx].x;
-            list[idx].y = gbase + (w0 & 0x7Fu) * rowbytes;
 #pragma unroll
             for (int t = 0; t < T; ++t) {
-                const uint32_t w = (t == 0) ? w0 : tok[(t - 1) * LN + idx];
-                const int b = (w >> 8) & 15;
+                const uint32_t ww = (t == 0) ? list[idx].x : tok[(t - 1) * LN + idx];
+                const int b = (ww >> 8) & 15;
                 if (b > 0) {
-                    const float xf = __half2float(__ushort_as_half((uint16_t)(w >> 16)));
+                    const float xf = __half2float(__ushort_as_half((uint16_t)(ww >> 16)));
                     Xp[t] += xf;
                     Pp[t] = fmaf(xf, (float)(0x80 >> b), Pp[t]);  // phi_b = 2^(7-b), phi_8 = 0
                 }
@@ -518,37 +469,61 @@ vmm_kernel(int K, int N, int Sx, int fused, const uint32_t* __restrict__ planes,
             Prun[t] += Pp[t];
         }
         app += n;
-        seg_p = p0 + n;
-        if (seg_p == seg_p1) {  // the warp's last row of this group: scale/zero chunks, X and Phi, next group
-            const int slot = segj & 15;
-            if (lane < 4)
-                list[(app + lane) & (LN - 1)] =
-                    make_uint2(ENTRY_SZ | (uint32_t)lane | ((uint32_t)slot << 16) | ((uint32_t)g << 8), 0u);
-            if (lane < T) {
-                float xs_ = 0.f, ps_ = 0.f;
+        seg_rows = seg_rows || n > 0;
+        if (seg_half == 0) {
+            seg_half = 1;
+        } else {  // the group is done for this warp: scale/zero chunks, X and Phi (if it had rows at all), next group
+            if (seg_rows) {
+                const int slot = segj & 15;
+                if (lane < 4)
+                    list[(app + lane) & (LN - 1)] =
+                        make_uint2(ENTRY_SZ | (uint32_t)lane | ((uint32_t)g << 8) | ((uint32_t)slot << 16), 0u);
+                if (lane < T) {
+                    float xs_ = 0.f, ps_ = 0.f;
 #pragma unroll
-                for (int t = 0; t < T; ++t)
-                    if (lane == t) {
-                        xs_ = Xrun[t];
-                        ps_ = Prun[t];
-                    }
-                xphi[slot * T + lane] = make_float2(xs_, ps_);
+                    for (int t = 0; t < T; ++t)
+                        if (lane == t) {
+                            xs_ = Xrun[t];
+                            ps_ = Prun[t];
+                        }
+                    xphi[slot * T + lane] = make_float2(xs_, ps_);
+                }
+                app += 4;
+                ++segj;
             }
 #pragma unroll
             for (int t = 0; t < T; ++t) Xrun[t] = Prun[t] = 0.f;
-            app += 4;
-            ++segj;
-            ++seg_g;
-            seg_p = 0;
+            seg_rows = false;
+            seg_half = 0;
+            seg_s = (g + 1) * GQ_G;
         }
         __syncwarp();
     };
 
-    // issues list entry iv into ring slot iv mod RING (one cp.async group, empty past the end of the list)
+    // issues list entry iv into ring slot iv mod RING (one cp.async group, empty past the end of the list; or bulk
+    // copies completing on the slot's mbarrier)
     auto issue_one = [&]() {
         if (iv < app) {
             const uint2 e = list[iv & (LN - 1)];
             const uint32_t so = (uint32_t)(iv & (RING - 1)) * SLOT_BYTES;
+            if (BULK) {
+                const uint32_t mb = mbar_s + (uint32_t)(iv & (RING - 1)) * 8;
+                if (!(e.x & ENTRY_SZ)) {
+                    const uint32_t b = (e.x >> 12) & 15;
+                    if (lane == 0) mbar_arrive_expect_tx(mb, b * segbytes);
+                    if ((uint32_t)lane < b && segbytes) bulk_g2s(ring_s + so + lane * 128, bulk_src + e.y, segbytes, mb);
+                } else {
+                    const uint32_t nact = (uint32_t)min(32, max(0, words - tile * 32));
+                    if (lane == 0) mbar_arrive_expect_tx(mb, nact * 32);
+                    if (active) {
+                        const size_t gn = (size_t)((e.x >> 8) & 0xFFu) * N + (size_t)word * 32 + 8 * (e.x & 3u);
+                        bulk_g2s(ring_s + so + lane * 16, scales + gn, 16, mb);
+                        bulk_g2s(ring_s + so + 512 + lane * 16, zeros + gn, 16, mb);
+                    }
+                }
+                ++iv;
+                return;
+            }
             if (!(e.x & ENTRY_SZ)) {
                 const int b = (e.x >> 12) & 15;
                 const uint8_t* src = lane_src + e.y;
@@ -568,7 +543,16 @@ vmm_kernel(int K, int N, int Sx, int fused, const uint32_t* __restrict__ planes,
             }
             ++iv;
         }
-        cp_async_commit();
+        if (!BULK) cp_async_commit();
+    };
+    // entry v has landed in its slot
+    auto wait_entry = [&](int v) {
+        if (BULK) {
+            mbar_wait(mbar_s + (uint32_t)(v & (RING - 1)) * 8, (uint32_t)(v / RING) & 1u);
+        } else {
+            cp_async_wait<RING - 3>();
+        }
+        __syncwarp();
     };
 
     GQ_STAMP();
@@ -577,6 +561,12 @@ vmm_kernel(int K, int N, int Sx, int fused, const uint32_t* __restrict__ planes,
 #pragma unroll 1
     for (int i = 0; i < RING - 2; ++i) issue_one();
     GQ_STAMP();
+    // the warp's accumulator tile starts at zero (cleared while the first rows are on their way)
+    {
+        float4* yz = reinterpret_cast<float4*>(yacc);
+#pragma unroll 1
+        for (int i = lane; i < T * YSLOT / 4; i += 32) yz[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    }
 
     float acc[T][32];
     float X[T], Phi[T];
@@ -710,8 +700,7 @@ vmm_kernel(int K, int N, int Sx, int fused, const uint32_t* __restrict__ planes,
                 constexpr int B = decltype(b_tag)::value;
 #pragma unroll 1
                 do {
-                    cp_async_wait<RING - 3>();
-                    __syncwarp();
+                    wait_entry(cv);
                     issue_one();
                     consume(b_tag, e, cv);
                     ++cv;
@@ -721,8 +710,7 @@ vmm_kernel(int K, int N, int Sx, int fused, const uint32_t* __restrict__ planes,
                                  : ((e >> 12) & 15) != 8 && ((e >> 12) & 15) != 4 && ((e >> 12) & 15) != 2));
             };
             if (e & ENTRY_SZ) {
-                cp_async_wait<RING - 3>();
-                __syncwarp();
+                wait_entry(cv);
                 issue_one();
                 const int L = (int)(e & 3u);
                 if (L == 0) chunk(integral_constant<int, 0>{}, e, cv);
@@ -740,7 +728,7 @@ vmm_kernel(int K, int N, int Sx, int fused, const uint32_t* __restrict__ planes,
             }
         }
     }
-    cp_async_wait<0>();
+    if (!BULK) cp_async_wait<0>();
     GQ_STAMP();
     __syncthreads();
     GQ_STAMP();
@@ -820,17 +808,17 @@ vmm_kernel(int K, int N, int Sx, int fused, const uint32_t* __restrict__ planes,
 __global__ void __launch_bounds__(256)
 vmm_reduce_kernel(const float* __restrict__ part, int S, int T, int N, float* __restrict__ y);
 
-template <int T, int VW, bool A16, int MODE>
+template <int T, int VW, bool A16, int MODE, bool BULK = false>
 static int launch_impl(const VmmArgs& a, const VmmPlan& pl) {
     using C = Cfg<T, VW>;
     const size_t smem = (size_t)C::BASE_BYTES + (MODE == MODE_SCHED ? 0 : (size_t)T * (a.K / GQ_G) * 16);
     // the attribute belongs to the device: set it on every launch (cheap, legal during stream capture)
-    if (cudaFuncSetAttribute(vmm_kernel<T, VW, A16, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) !=
+    if (cudaFuncSetAttribute(vmm_kernel<T, VW, A16, MODE, BULK>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) !=
         cudaSuccess)
         return GRINQH_ERR_CUDA;
     dim3 grid(pl.col_tiles, pl.Sx);
     const cudaError_t e =
-        launch_pdl(vmm_kernel<T, VW, A16, MODE>, grid, dim3(C::NT), smem, a.st, a.K, a.N, pl.Sx, a.fused, a.planes,
+        launch_pdl(vmm_kernel<T, VW, A16, MODE, BULK>, grid, dim3(C::NT), smem, a.st, a.K, a.N, pl.Sx, a.fused, a.planes,
                    (const __half*)a.scales, (const __half*)a.zeros, a.gsched, a.gcnt_ge, a.xraw, a.cp,
                    (float*)((char*)a.workspace + TICKET_BYTES), (int*)a.workspace, a.y);
     return e == cudaSuccess ? GRINQH_OK : GRINQH_ERR_CUDA;
