@@ -3,9 +3,10 @@
 
 Workload (N = 1): BASELINE.json configs[1] — one Llama-3-8B-shaped layer, batch 1, avg 4 bits:
 7 projections (q,k,v,o,gate,up,down), 4 distinct input vectors (q/k/v and gate/up share one).
-A "step" = one pass of the per-step hot path over one layer: 4 x grinqh_assign + 4 x grinqh_vmm (q|k|v and
-gate|up concatenated along N; the deterministic split-K second pass runs inside the VMM launch).  The same step
-with one launch per projection (7 VMMs) is reported under "per_projection".  grinqh_pack is offline (once per weight) and reported separately under "pack".
+A "step" = one pass of the per-step hot path over one layer: 4 x grinqh_vmm_rank — the rank assignment of the input
+vector, the selective plane fetch and the deterministic split-K second pass all inside ONE launch per input vector
+(q|k|v and gate|up concatenated along N).  The same step as 4 x grinqh_assign + 4 x grinqh_vmm ("two_kernel_form"),
+with one launch per projection ("per_projection") and with the paper's threshold assignment are reported beside it.  grinqh_pack is offline (once per weight) and reported separately under "pack".
 The timed loop rotates over LAYERS distinct packed layers (> L2) so every step streams from HBM.
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--mix 4] [--layers 4]
@@ -24,10 +25,19 @@ import time
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
-# DRAM bytes moved by the 4 VMM launches of one step, from the committed ncu --set full capture (profiles/r01_kernels.md):
-# 116.26 MB read + 0.67 MB written, against 116.23 MB algorithmic.  Only the default mix was captured.
-NCU_TRAFFIC_BYTES_PER_STEP = {"4": 116.94e6}
-METRIC = "us per decode step of one Llama-3-8B-shaped layer (4 assigns + the 7 projections as bit-planar VMMs), batch 1"
+METRIC = "us per decode step of one Llama-3-8B-shaped layer (4 rank assignments + the 7 projections as bit-planar VMMs), batch 1"
+
+
+def _committed_traffic(mix):
+    """dram__bytes_read.sum + dram__bytes_write.sum of the step's launches from the committed ncu capture
+    (profiles/r02_traffic.json, written from an `ncu --set full` run of this command; it names the commit it was
+    taken on).  None when no capture of this mix is committed: the value is never made up."""
+    p = os.path.join(ROOT, "profiles", "r02_traffic.json")
+    try:
+        d = json.load(open(p))
+        return d["bytes_per_step"].get(mix), d.get("captured_on")
+    except Exception:
+        return None, None
 UNIT = "us"
 
 
@@ -118,7 +128,7 @@ class OracleLayerSample:
     `cols_per_proj` output columns (all K rows) + the 4 assignments.  Packing the sample is offline
     (not timed).  run() returns the seconds one sampled step took; `fraction` scales it to the full layer."""
 
-    def __init__(self, mix_name: str, seed: int, cols_per_proj: int):
+    def __init__(self, mix_name: str, seed: int, cols_per_proj: int = 1 << 30):
         import oracle
         from paper_2606_23419_b200 import synth
         self.oracle, self.synth = oracle, synth
@@ -132,9 +142,13 @@ class OracleLayerSample:
             full_w += K * N
             samp_w += K * n
         self.fraction = samp_w / full_w
-        self.desc = (f"oracle assign x4 + oracle vmm (fp64, 1 thread) on the first {cols_per_proj} output columns of "
-                     f"each of the 7 projections ({samp_w / 1e6:.2f}M of {full_w / 1e6:.1f}M weights), "
-                     f"time scaled by the weight ratio")
+        if samp_w == full_w:
+            self.desc = ("oracle assign x4 + oracle vmm (fp64, 1 thread) on the FULL layer step: all output columns of "
+                         f"the 7 projections ({full_w / 1e6:.1f}M weights), no scaling")
+        else:
+            self.desc = (f"oracle assign x4 + oracle vmm (fp64, 1 thread) on the first {cols_per_proj} output columns of "
+                         f"each of the 7 projections ({samp_w / 1e6:.2f}M of {full_w / 1e6:.1f}M weights), "
+                         f"time scaled by the weight ratio")
 
     def run(self) -> float:
         oracle, synth = self.oracle, self.synth
@@ -149,30 +163,40 @@ class OracleLayerSample:
         return time.perf_counter() - t0
 
 
+WORKLOAD = ("llama3-8b-layer (BASELINE.json configs[1]): 4096->4096 x2 (q,o), 4096->1024 x2 (k,v), "
+            "4096->14336 x2 (gate,up), 14336->4096 (down); batch 1; per-step rank assignment")
+
+
 def run_reference(args):
+    """The oracle as it stands on the host cores.  A full layer step takes ~4 s on one core: when steps + warmup of
+    them fit in ~150 s every step IS the full step (no scaling); otherwise each step is the first `cols` output
+    columns of every projection and the time is scaled by the weight ratio (said in the line)."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
     from paper_2606_23419_b200 import synth
-    # size the per-step sample so that the whole run stays within ~2 minutes (about 25 ns per weight)
-    budget = 120.0 / max(1, args.steps + args.warmup)
+    n = max(1, args.steps + args.warmup)
     rows = sum(K for _, K, _ in synth.LLAMA3_8B_LAYER)
-    cols = int(budget / (rows * 32 * 25e-9)) * 32
-    cols = max(32, min(1024, cols))
-    sample = OracleLayerSample(args.mix, args.seed, cols)
+    if n * 4.5 <= 150.0:
+        sample = OracleLayerSample(args.mix, args.seed)
+    else:
+        budget = 120.0 / n                                # about 25 ns per weight
+        cols = max(32, min(1024, int(budget / (rows * 32 * 25e-9)) * 32))
+        sample = OracleLayerSample(args.mix, args.seed, cols)
     times = []
     for i in range(args.warmup + args.steps):
         t = sample.run()
         if i >= args.warmup:
-            times.append(t / sample.fraction)
-    us = 1e6 * sum(times) / len(times)
+            times.append(t)
+    sec = sum(times) / len(times)
+    us = 1e6 * sec / sample.fraction
     line = {
         "impl": "reference", "metric": METRIC, "value": us, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": us / 1e3, "higher_is_better": False, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": "llama3-8b-layer (BASELINE.json configs[1]), batch 1",
-                   "avg_bits": synth.mix_avg_bits(synth.MIXES[args.mix]), "mix": args.mix},
-        "cpu_baseline": {"value": us, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample.desc},
+        "config": {"workload": WORKLOAD, "avg_bits": synth.mix_avg_bits(synth.MIXES[args.mix]), "mix": args.mix},
+        "cpu_baseline": {"value": us, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample.desc,
+                         "sample_fraction": sample.fraction, "seconds_per_timed_step_as_run": sec},
         "e2e": {"value": us, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
@@ -256,51 +280,42 @@ def run_native(args):
     ws = gq.grinqh_vmm_workspace(T, Kw, Nw, dev)
     x_stage = {n: torch.empty((T, K), dtype=torch.float16, device=dev) for n, K in in_dims.items()}
 
-    def step_device(l):          # the timed step: 4 assigns + 4 VMM launches (qkv and gate/up concatenated)
+    def step_device(l):          # the timed step: the rank assignment inside the VMM launch, 4 launches
+        for name, K, N, inp in fused:
+            gq.grinqh_vmm_rank(x_dev[l][inp], counts[K], packed[l][name], y_dev[l][name], ws)
+
+    def step_two_kernel(l):      # the same step as 4 x grinqh_assign + 4 x grinqh_vmm (round 1's form)
         for name, K, N, inp in fused:
             gq.grinqh_assign(x_dev[l][inp], counts[K], assigns[l][inp])
             gq.grinqh_vmm(packed[l][name], assigns[l][inp], y_dev[l][name], ws)
 
-    def step_split(l):           # the same step with one launch per projection: 4 assigns + 7 VMMs
-        seen = set()
+    def step_split(l):           # one launch per projection: 7 x grinqh_vmm_rank
         for name, K, N, inp in split:
-            if inp not in seen:
-                gq.grinqh_assign(x_dev[l][inp], counts[K], assigns[l][inp])
-                seen.add(inp)
-            gq.grinqh_vmm(packed_split[l][name], assigns[l][inp], y_dev[l][name], ws)
+            gq.grinqh_vmm_rank(x_dev[l][inp], counts[K], packed_split[l][name], y_dev[l][name], ws)
 
     # threshold form: thetas calibrated offline on 8 synthetic vectors per input
     thetas = {n: gq.grinqh_calibrate_thresholds(
         torch.from_numpy(np.concatenate([synth.make_x(1, K, 7000 + 10 * i + s, "normal") for s in range(8)], axis=0)),
         counts[K]) for i, (n, K) in enumerate(in_dims.items())}
 
-    def step_thresholds(l):      # the same step with the paper's threshold assignment instead of the rank form
-        for name, K, N, inp in fused:
-            gq.grinqh_assign_thresholds(x_dev[l][inp], thetas[inp], assigns[l][inp])
-            gq.grinqh_vmm(packed[l][name], assigns[l][inp], y_dev[l][name], ws)
-
-    def step_thresholds_fused(l):  # ... and with that assignment made inside the VMM launch: 4 launches per step
+    def step_thresholds_fused(l):  # the paper's threshold assignment made inside the VMM launch: 4 launches per step
         for name, K, N, inp in fused:
             gq.grinqh_vmm_thresholds(x_dev[l][inp], thetas[inp], packed[l][name], y_dev[l][name], ws)
 
-    def step_rank_fused(l):      # the rank assignment made inside the VMM launch: 4 launches per step
-        for name, K, N, inp in fused:
-            gq.grinqh_vmm_rank(x_dev[l][inp], counts[K], packed[l][name], y_dev[l][name], ws)
-
-    def step_main_only(l):       # the dominant kernel alone: the 4 VMM launches (assignments already on the device)
+    def step_sched_only(l):      # the VMM launches alone, on schedules already made by grinqh_assign
         for name, K, N, inp in fused:
             gq.grinqh_vmm(packed[l][name], assigns[l][inp], y_dev[l][name], ws)
 
     def step_host(l, force_copies=False):
         for name, K, N, inp in fused:
-            gq.grinqh_decode_host(x_host[l][inp], counts[K], packed[l][name], assigns[l][inp], x_stage[inp],
-                                  y_dev[l][name], ws, y_host[l][name], reuse_assignment=False,
-                                  force_copies=force_copies)
+            gq.grinqh_decode_host(x_host[l][inp], counts[K], packed[l][name], x_stage[inp], y_dev[l][name], ws,
+                                  y_host[l][name], force_copies=force_copies)
 
     stream = torch.cuda.Stream(device=dev)
     with torch.cuda.stream(stream):
-        for l in range(L):          # eager warm-up (also configures kernel attributes before capture)
+        for l in range(L):          # eager warm-up
             step_device(l)
+            step_two_kernel(l)
             step_host(l)
             if packed_split:
                 step_split(l)
@@ -315,11 +330,6 @@ def run_native(args):
                 graphs.append(g)
             return graphs
 
-        g_dev = capture(step_device)
-        g_main = capture(step_main_only)
-        g_host = capture(step_host)
-        g_split = capture(step_split) if packed_split else None
-
         def barrier():
             if world > 1:
                 import torch.distributed as dist
@@ -327,6 +337,8 @@ def run_native(args):
             torch.cuda.synchronize()
 
         def timed(graphs, steps, sync_each=False):
+            for i in range(3):
+                graphs[i % L].replay()
             a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             barrier()
             a.record(stream)
@@ -336,54 +348,31 @@ def run_native(args):
                     stream.synchronize()
             b.record(stream)
             barrier()
-            return a.elapsed_time(b)
+            return a.elapsed_time(b) * 1e3 / steps   # us per step
 
+        g_dev = capture(step_device)
         for i in range(max(args.warmup, 3)):
             g_dev[i % L].replay()
         sampler = ClockSampler(local)
         sampler.start()
-        ms_total = timed(g_dev, args.steps)
+        us_step = timed(g_dev, args.steps)
         clocks = sampler.stop()
-        for i in range(3):
-            g_main[i % L].replay()
-        ms_main = timed(g_main, args.steps)
-        for i in range(3):
-            g_host[i % L].replay()
-        ms_host = timed(g_host, args.steps, sync_each=True)
-        g_hostc = capture(lambda l: step_host(l, True))
-        for i in range(3):
-            g_hostc[i % L].replay()
-        ms_hostc = timed(g_hostc, max(50, args.steps // 4), sync_each=True) * args.steps / max(50, args.steps // 4)
-        step_thresholds(0)
-        stream.synchronize()
-        g_thr = capture(step_thresholds)
-        for i in range(3):
-            g_thr[i % L].replay()
-        ms_thr = timed(g_thr, args.steps)
+        us_host = timed(capture(step_host), args.steps, sync_each=True)
+        n_c = max(50, args.steps // 4)
+        us_hostc = timed(capture(lambda l: step_host(l, True)), n_c, sync_each=True)
+        us_two = timed(capture(step_two_kernel), args.steps)
+        us_sched = timed(capture(step_sched_only), args.steps)
         step_thresholds_fused(0)
         stream.synchronize()
-        g_thrf = capture(step_thresholds_fused)
-        for i in range(3):
-            g_thrf[i % L].replay()
-        ms_thrf = timed(g_thrf, args.steps)
-        step_rank_fused(0)
-        stream.synchronize()
-        g_rf = capture(step_rank_fused)
-        for i in range(3):
-            g_rf[i % L].replay()
-        ms_rf = timed(g_rf, args.steps)
-        thr_bits = float(np.mean([assigns[0][n].bits.float().mean().item() for n in in_dims]))
-        for l in range(L):       # leave the rank-form assignments in the buffers (byte accounting below)
+        us_thrf = timed(capture(step_thresholds_fused), args.steps)
+        us_split = timed(capture(step_split), args.steps) if packed_split else 0.0
+        for l in range(L):       # the rank-form assignments (byte accounting below)
             for n, K in in_dims.items():
                 gq.grinqh_assign(x_dev[l][n], counts[K], assigns[l][n])
         stream.synchronize()
-        ms_split = None
-        if g_split:
-            for i in range(3):
-                g_split[i % L].replay()
-            ms_split = timed(g_split, args.steps)
 
-    ms_total, ms_main, ms_host, ms_split = max_over_ranks([ms_total, ms_main, ms_host, ms_split or 0.0], dev)
+    us_step, us_host, us_hostc, us_two, us_sched, us_thrf, us_split = max_over_ranks(
+        [us_step, us_host, us_hostc, us_two, us_sched, us_thrf, us_split], dev)
 
     # ---- algorithmic bytes of the VMM launches of one step (measured widths; SURVEY.md 8d / DESIGN.md)
     step_bytes, plane_bytes = 0, 0
@@ -395,58 +384,58 @@ def run_native(args):
         plane_bytes += (N // 8) * sb
         per_vmm.append({"launch": name, "K": K, "N": N, "alg_bytes": b})
     peak, peak_src = _peaks()
-    us_step = ms_total * 1e3 / args.steps
-    us_main = ms_main * 1e3 / args.steps
-    us_host = ms_host * 1e3 / args.steps
-    achieved = step_bytes / (us_main * 1e-6) / 1e9  # GB/s over the VMM launches of a step
+    achieved = step_bytes / (us_step * 1e-6) / 1e9  # GB/s over the launches of a step (assignment included)
+    traffic, traffic_on = _committed_traffic(args.mix)
 
     h2d = sum(T * K * 2 for K in in_dims.values())
     d2h = sum(T * N * 4 for _, _, N, _ in fused)
     weights = sum(K * N for _, K, N, _ in fused)
     line = {
-        "metric": METRIC, "value": us_step / world, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "metric": METRIC, "value": us_step, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": us_step / 1e3, "higher_is_better": False, "scaling": "weak",
         "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-        "config": {"workload": "llama3-8b-layer (BASELINE.json configs[1]): 4096->4096 x2 (q,o), 4096->1024 x2 (k,v), "
-                               "4096->14336 x2 (gate,up), 14336->4096 (down); batch 1; per-step rank assignment",
-                   "launches": "4 x grinqh_assign + 4 x grinqh_vmm per step: q|k|v and gate|up are concatenated along N "
-                               "(same input vector, per-column quantiser), the split-K second pass runs inside the VMM launch",
+        "config": {"workload": WORKLOAD,
+                   "launches": "4 x grinqh_vmm_rank per step: the rank assignment (one shared-memory histogram select per "
+                               "CTA), the selective plane fetch and the deterministic split-K second pass in ONE launch per "
+                               "input vector; q|k|v and gate|up are concatenated along N (same input vector, per-column "
+                               "quantiser)",
                    "avg_bits": avg_bits, "mix": args.mix, "group": 128, "tokens": T,
                    "l2": f"timed loop rotates over {L} distinct packed layers "
                          f"({L * weights / 1e6:.0f} MB of planes > 126 MB L2); one CUDA graph per layer",
-                   "replicas": "replicas only (no data-path collective)" if world > 1 else "single GPU"},
+                   "replicas": ("replicas only (no data-path collective): value = slowest rank's us per step"
+                                if world > 1 else "single GPU")},
         "clocks": clocks,
-        "e2e": {"value": us_host / world, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                "how": "grinqh_decode_host per launch, stream sync per step: x is read from the pinned HOST buffer by the "
-                       "assignment kernel and y is written into the pinned HOST buffer by the VMM's second pass (host-mapped "
-                       "access, no copy nodes); the bytes cross PCIe inside the timed region every step",
-                "value_with_copy_nodes": ms_hostc * 1e3 / args.steps / world},
-        "gpu_launches": args.steps * 2 * len(fused),
+        "e2e": {"value": us_host, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                "how": "grinqh_decode_host per launch, stream sync per step: x is copied from the pinned HOST buffer with "
+                       "cudaMemcpyAsync, the VMM's second pass writes y into the pinned HOST buffer (host-mapped access); "
+                       "the bytes cross PCIe inside the timed region every step",
+                "value_with_y_copy_nodes": us_hostc},
+        "gpu_launches": args.steps * len(fused),
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": NCU_TRAFFIC_BYTES_PER_STEP.get(args.mix),
-                     "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum over the step's VMM launches, "
-                                       "ncu --set full capture of this command (profiles/r01_kernels.md)",
-                     "kernel": f"vmm_main_kernel<T=1, 16 warps, 16-byte copies, fused second pass> ({len(fused)} launches per step)",
+                     "traffic": traffic,
+                     "traffic_source": (f"dram__bytes_read.sum + dram__bytes_write.sum of the step's launches, committed "
+                                        f"ncu --set full capture (profiles/r02_traffic.json, taken on {traffic_on})"
+                                        if traffic else "no committed capture for this mix"),
+                     "kernel": f"vmm_kernel<T=1, MODE_RANK> ({len(fused)} launches per step = the whole step)",
                      "alg_bytes_per_step": step_bytes, "plane_bytes_per_step": plane_bytes,
-                     "us_per_step_main_only": us_main, "peak_source": peak_src},
+                     "us_per_step_vmm_on_ready_schedules": us_sched,
+                     "frac_vmm_on_ready_schedules": step_bytes / (us_sched * 1e-6) / 1e9 / peak,
+                     "peak_source": peak_src},
         "pack": {"GBps": pack_bytes / (pack_ms * 1e-3) / 1e9, "ms_per_layer": pack_ms / L},
         "per_vmm": per_vmm,
+        "steps_per_s_total": world / (us_step * 1e-6),
+        "two_kernel_form": {"value": us_two, "unit": UNIT,
+                            "what": "the same step as 4 x grinqh_assign + 4 x grinqh_vmm (8 launches)"},
+        "threshold_assignment_fused": {"value": us_thrf, "unit": UNIT,
+                                       "what": "the paper's threshold assignment (PAPER.md:61-65, thetas calibrated on 8 "
+                                               "synthetic vectors) made inside the VMM launch (grinqh_vmm_thresholds)"},
     }
-    line["threshold_assignment"] = {"value": max_over_ranks([ms_thr], dev)[0] * 1e3 / args.steps, "unit": UNIT,
-                                    "avg_bits_measured": thr_bits,
-                                    "what": "same step with grinqh_assign_thresholds (the paper's run-time form, thetas "
-                                            "calibrated on 8 synthetic vectors) instead of the rank assignment"}
-    line["threshold_assignment_fused"] = {"value": max_over_ranks([ms_thrf], dev)[0] * 1e3 / args.steps, "unit": UNIT,
-                                          "what": "the same with the threshold assignment made inside the VMM launch "
-                                                  "(grinqh_vmm_thresholds): 4 launches per step"}
-    line["rank_assignment_fused"] = {"value": max_over_ranks([ms_rf], dev)[0] * 1e3 / args.steps, "unit": UNIT,
-                                     "what": "the rank assignment made inside the VMM launch (grinqh_vmm_rank): 4 launches per step"}
-    if ms_split:
-        line["per_projection"] = {"value": ms_split * 1e3 / args.steps, "unit": UNIT,
-                                  "what": "same step with one VMM launch per projection (4 assigns + 7 VMMs)"}
+    if us_split:
+        line["per_projection"] = {"value": us_split, "unit": UNIT,
+                                  "what": "same step with one grinqh_vmm_rank launch per projection (7 launches)"}
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        sample = OracleLayerSample(args.mix, args.seed, 1024)
-        t = min(sample.run() for _ in range(3))
+        sample = OracleLayerSample(args.mix, args.seed)   # the full layer step, as it stands, on one host core
+        t = min(sample.run() for _ in range(2))
         line["cpu_baseline"] = {"value": 1e6 * t / sample.fraction, "unit": UNIT, "cores": 1, "kind": "oracle",
                                 "sample": sample.desc}
     if rank == 0:
@@ -513,13 +502,14 @@ def run_sweep(args):
                 gq.grinqh_assign(x, counts, a)
                 torch.cuda.synchronize()
                 union_bits = float(a.bits_union.sum().item()) / K
-                us_vmm = time_graph(lambda: [gq.grinqh_vmm(w, a, y, ws) for w in packed], copies)
+                us_vmm = time_graph(lambda: [gq.grinqh_vmm_rank(x, counts, w, y, ws) for w in packed], copies)
+                us_sched = time_graph(lambda: [gq.grinqh_vmm(w, a, y, ws) for w in packed], copies)
                 us_asg = time_graph(lambda: [gq.grinqh_assign(x, counts, a) for _ in range(8)], 8)
                 ab = alg_bytes(K, N, T, int(a.bits_union.sum().item()))
                 rec = {"model": model, "K": K, "N": N, "T": T, "mix": mix,
                        "avg_bits_per_token": synth.mix_avg_bits(synth.MIXES[mix]), "union_bits": union_bits,
-                       "us_vmm": us_vmm, "us_assign": us_asg, "alg_MB": ab / 1e6,
-                       "GBps": ab / us_vmm / 1e3, "frac_of_measured_hbm": ab / us_vmm / 1e3 / peak}
+                       "us_vmm_rank": us_vmm, "us_vmm_on_ready_schedule": us_sched, "us_assign": us_asg,
+                       "alg_MB": ab / 1e6, "GBps": ab / us_vmm / 1e3, "frac_of_measured_hbm": ab / us_vmm / 1e3 / peak}
                 pts.append((union_bits, us_vmm))
                 print("SWEEP " + json.dumps(rec), flush=True)
             n = len(pts)
@@ -528,7 +518,7 @@ def run_sweep(args):
             a0 = my - c * mx
             ss_res = sum((p[1] - (a0 + c * p[0])) ** 2 for p in pts)
             ss_tot = sum((p[1] - my) ** 2 for p in pts)
-            print("SWEEP " + json.dumps({"model": model, "K": K, "N": N, "T": T, "fit": "us_vmm = a + c * union_bits",
+            print("SWEEP " + json.dumps({"model": model, "K": K, "N": N, "T": T, "fit": "us_vmm_rank = a + c * union_bits",
                                          "a_us": a0, "c_us_per_bit": c, "r2": 1 - ss_res / ss_tot}), flush=True)
         del packed
         torch.cuda.empty_cache()
@@ -571,11 +561,14 @@ def run_decode_step(args):
     for mix in ("2", "3", "4", "8"):
         counts = {K: gq.grinqh_mix_to_counts(K, synth.MIXES[mix]) for K in set(in_dims.values())}
 
-        def step():
+        def step():            # 128 launches: the rank assignment inside every VMM launch
             for l in range(NL):
                 for name, K, N, inp in fused:
-                    gq.grinqh_assign(xs[l][inp], counts[K], assigns[l][inp])
-                    gq.grinqh_vmm(packed[l][name], assigns[l][inp], ys[l][name], ws)
+                    gq.grinqh_vmm_rank(xs[l][inp], counts[K], packed[l][name], ys[l][name], ws)
+
+        for l in range(NL):    # (the assignments themselves, for the byte accounting below)
+            for n_, K_ in in_dims.items():
+                gq.grinqh_assign(xs[l][n_], counts[K_], assigns[l][n_])
 
         with torch.cuda.stream(stream):
             step()
@@ -622,10 +615,10 @@ def run_decode_step(args):
         us_thr = a2.elapsed_time(b2) * 1e3 / reps
         nbytes = sum(alg_bytes(K, N, T, int(assigns[l][inp].bits_union.sum().item()))
                      for l in range(NL) for name, K, N, inp in fused)
-        print("DECODE " + json.dumps({"workload": "32-layer llama3-8b-shaped decode step, 256 launches in one CUDA graph",
+        print("DECODE " + json.dumps({"workload": "32-layer llama3-8b-shaped decode step, 128 grinqh_vmm_rank launches in one CUDA graph",
                                       "mix": mix, "avg_bits": synth.mix_avg_bits(synth.MIXES[mix]), "us_per_decode_step": us,
                                       "us_per_decode_step_thresholds_fused": us_thr,
-                                      "alg_GB": nbytes / 1e9, "GBps_incl_assign": nbytes / us / 1e3,
+                                      "alg_GB": nbytes / 1e9, "GBps": nbytes / us / 1e3,
                                       "frac_of_measured_hbm": nbytes / us / 1e3 / peak}), flush=True)
 
 

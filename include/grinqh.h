@@ -56,7 +56,7 @@ typedef enum {
 
 #define GRINQH_GROUP 128
 #define GRINQH_MAX_T 4
-#define GRINQH_MAX_K 32768      /* assignment runs in one CTA; keys + histogram must fit */
+#define GRINQH_MAX_K 32768      /* the 15-bit key histogram and one token's keys live in one CTA's shared memory */
 #define GRINQH_GCNT_STRIDE 16   /* bytes per group in gcnt_ge (entries 0..9 used)        */
 
 /* Static strings, never freed. */
@@ -120,7 +120,9 @@ int grinqh_unpack(const uint32_t* planes, const void* scales_f16, const void* ze
  *                                        the i-th row of group g's list, r = grows[128 g + i], k = 128 g + r:
  *                                          bits 0..7 r | 8..11 bits[t][k] | 12..15 bits_union[k] | 16..31 x[t][k] (fp16 pattern)
  *                                        a pure re-indexing of the outputs above (bit-exact against the oracle's)
- *   workspace   dev   >= grinqh_assign_workspace_bytes(T, K) bytes, 16-byte aligned
+ *   workspace   dev   unused: grinqh_assign_workspace_bytes returns 0 (everything lives in shared memory); the
+ *                     arguments are kept for ABI stability and may be NULL / 0
+ * Any of the seven output pointers may be NULL: that output is skipped (grinqh_vmm reads gsched only).
  */
 size_t grinqh_assign_workspace_bytes(int T, int K);
 int grinqh_assign(const void* x_f16, int T, int K, const uint32_t counts[9],
@@ -148,12 +150,13 @@ int grinqh_calibrate_thresholds(const void* x_host_f16, int S, int K, const uint
 
 /*
  * grinqh_vmm — per projection (PAPER.md:85 reconstruction, :51 selective fetch).
- * ONE launch: split-K main kernel (warps walk the per-group schedule and fetch only planes j < bits_union[k] of
- * row k) whose last-finishing CTA per column tile runs the deterministic second pass: it sums the tile's split-K
+ * ONE launch: split-K main kernel (warps walk their slots of the per-group schedule and fetch only planes
+ * j < bits_union[k] of row k) whose last-finishing CTA per column tile runs the deterministic second pass: it sums the tile's split-K
  * partials in the fixed order s = 0..S-1 (the result does not depend on which CTA is last).  fp32 accumulation.
  * For T > 1 each token is truncated to its own bits[t][k]; y[t] equals the T = 1 result of token t alone.
  * The activations enter through gsched (x values, widths and row order of the assignment).
- *   gsched, gcnt_ge   dev   as written by grinqh_assign for this [T, K] input
+ *   gsched, gcnt_ge   dev   as written by grinqh_assign for this [T, K] input (gcnt_ge is not read any more:
+ *                           rows with b = 0 are recognised from their schedule entries; any non-NULL pointer will do)
  *   y          dev  [T, N] fp32, written
  *   workspace  dev  >= grinqh_vmm_workspace_bytes(T, K, N) bytes, 16-byte aligned.  Its first 16 KB hold the
  *                   per-tile tickets: call grinqh_vmm_workspace_init ONCE after allocating it (and again only
@@ -199,28 +202,21 @@ int grinqh_vmm_rank(const void* x_f16, int T, int K, int N, int group, const uin
                     float* y, void* workspace, size_t workspace_bytes, void* stream);
 
 /*
- * Host-buffer decode call (the end-to-end entry): x comes from HOST memory, grinqh_assign + grinqh_vmm run, y ends
- * in HOST memory, all enqueued on `stream`.  With pinned (page-locked) buffers the kernels access host memory
- * directly (x is read once by the assignment, y is written by the VMM's second pass): no copy nodes.  With pageable
- * buffers, or GRINQH_FORCE_COPIES, x is staged through x_dev_f16 and y through y_dev with cudaMemcpyAsync.  The packed weights stay
- * resident on the device.  The caller synchronises the stream before reading
- * y_host.
- *   x_host_f16  HOST [T, K] fp16       y_host  HOST [T, N] fp32
+ * Host-buffer decode call (the end-to-end entry): x comes from HOST memory, the rank assignment and the VMM run in
+ * one launch (grinqh_vmm_rank), y ends in HOST memory, all enqueued on `stream`.  x is staged with one
+ * cudaMemcpyAsync (every CTA reads all of x for its rank selection).  With a pinned (page-locked) y_host the VMM's
+ * second pass writes y straight into host memory; a pageable buffer, or GRINQH_FORCE_COPIES, is staged through y_dev
+ * with cudaMemcpyAsync.  The packed weights stay resident on the device.  The caller synchronises the stream before
+ * reading y_host.  All arguments are validated before anything is enqueued.
+ *   x_host_f16  HOST [T, K] fp16       y_host  HOST [T, N] fp32       counts HOST [9], sum = K
  *   x_dev_f16   dev  [T, K] fp16 staging, y_dev dev [T, N] fp32 staging
- *   assign_ws / vmm_ws: device workspaces as above
- *   flags       GRINQH_REUSE_ASSIGNMENT: the assignment buffers already hold this x
- *               (a previous call for a projection that consumes the same input vector — q/k/v, gate/up);
- *               skip the host->device copy and grinqh_assign.
+ *   vmm_ws      dev  workspace of grinqh_vmm_workspace_bytes(T, K, N) bytes (tickets initialised)
  */
-#define GRINQH_REUSE_ASSIGNMENT 1
-#define GRINQH_FORCE_COPIES 2   /* always stage through x_dev_f16 / y_dev with cudaMemcpyAsync */
+#define GRINQH_FORCE_COPIES 2   /* always stage y through y_dev with cudaMemcpyAsync */
 int grinqh_decode_host(const void* x_host_f16, int T, int K, int N, int group,
                        const uint32_t counts[9],
                        const uint32_t* planes, const void* scales_f16, const void* zeros_f16,
-                       void* x_dev_f16, uint8_t* bits, uint8_t* bits_union, int32_t* rows, int32_t* cnt_ge,
-                       uint8_t* grows, uint8_t* gcnt_ge, uint32_t* gsched,
-                       void* assign_ws, size_t assign_ws_bytes,
-                       float* y_dev, void* vmm_ws, size_t vmm_ws_bytes,
+                       void* x_dev_f16, float* y_dev, void* vmm_ws, size_t vmm_ws_bytes,
                        float* y_host, int flags, void* stream);
 
 #ifdef __cplusplus

@@ -59,8 +59,7 @@ _lib.grinqh_vmm_main.argtypes = _VMM_COMMON + [_vp, _sz, _vp]
 _lib.grinqh_vmm_reduce.restype = _i
 _lib.grinqh_vmm_reduce.argtypes = [_i, _i, _i, _vp, _vp, _sz, _vp]
 _lib.grinqh_decode_host.restype = _i
-_lib.grinqh_decode_host.argtypes = [_vp, _i, _i, _i, _i, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp,
-                                    _vp, _vp, _sz, _vp, _vp, _sz, _vp, _i, _vp]
+_lib.grinqh_decode_host.argtypes = [_vp, _i, _i, _i, _i, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _sz, _vp, _i, _vp]
 
 EXPORTS = ("grinqh_status_string", "grinqh_version", "grinqh_mix_to_counts", "grinqh_pack", "grinqh_unpack",
            "grinqh_assign_workspace_bytes", "grinqh_assign", "grinqh_assign_thresholds",
@@ -259,16 +258,15 @@ def grinqh_vmm_reduce(T: int, K: int, N: int, y: torch.Tensor, workspace: torch.
            "grinqh_vmm_reduce")
 
 
-def grinqh_decode_host(x_host: torch.Tensor, counts, w: Packed, a: Assignment, x_dev: torch.Tensor,
-                       y_dev: torch.Tensor, workspace: torch.Tensor, y_host: torch.Tensor,
-                       reuse_assignment: bool = False, force_copies: bool = False, stream=None):
-    """HOST x [T, K] fp16 (pinned) -> HOST y [T, N] fp32 (pinned); weights stay on the device.  Enqueue only."""
+def grinqh_decode_host(x_host: torch.Tensor, counts, w: Packed, x_dev: torch.Tensor, y_dev: torch.Tensor,
+                       workspace: torch.Tensor, y_host: torch.Tensor, force_copies: bool = False, stream=None):
+    """HOST x [T, K] fp16 -> HOST y [T, N] fp32 (rank assignment inside the VMM launch); weights stay on the device.
+    Enqueue only."""
     T, K = x_host.shape
     if x_host.is_cuda or y_host.is_cuda:
         raise GrinqhError("grinqh_decode_host takes HOST x and y")
     _check(_lib.grinqh_decode_host(
         x_host.data_ptr(), T, K, w.N, GROUP, _counts(counts), w.planes.data_ptr(), w.scales.data_ptr(),
-        w.zeros.data_ptr(), x_dev.data_ptr(), a.bits.data_ptr(), a.bits_union.data_ptr(), a.rows.data_ptr(),
-        a.cnt_ge.data_ptr(), a.grows.data_ptr(), a.gcnt_ge.data_ptr(), a.gsched.data_ptr(), None, 0, y_dev.data_ptr(),
-        workspace.data_ptr(), workspace.numel() * workspace.element_size(), y_host.data_ptr(),
-        (1 if reuse_assignment else 0) | (2 if force_copies else 0), _stream(stream)), "grinqh_decode_host")
+        w.zeros.data_ptr(), x_dev.data_ptr(), y_dev.data_ptr(), workspace.data_ptr(),
+        workspace.numel() * workspace.element_size(), y_host.data_ptr(), 2 if force_copies else 0, _stream(stream)),
+        "grinqh_decode_host")

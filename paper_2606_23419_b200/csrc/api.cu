@@ -20,7 +20,7 @@ extern "C" const char* grinqh_status_string(int status) {
     }
 }
 
-extern "C" int grinqh_version(void) { return 200; /* 0.2.0: gsched schedule, fused second pass, threshold assignment */ }
+extern "C" int grinqh_version(void) { return 300; /* 0.3.0: grinqh_vmm_rank, slot-striped VMM, histogram select */ }
 
 // PAPER.md:262-266 (Eq. 1): precision distribution P -> integer row counts; reading #3.
 extern "C" int grinqh_mix_to_counts(int K, const double frac[9], uint32_t counts[9]) {
@@ -87,43 +87,40 @@ extern "C" int grinqh_calibrate_thresholds(const void* x_host_f16, int S, int K,
 
 extern "C" int grinqh_decode_host(const void* x_host_f16, int T, int K, int N, int group, const uint32_t counts[9],
                                   const uint32_t* planes, const void* scales_f16, const void* zeros_f16,
-                                  void* x_dev_f16, uint8_t* bits, uint8_t* bits_union, int32_t* rows,
-                                  int32_t* cnt_ge, uint8_t* grows, uint8_t* gcnt_ge, uint32_t* gsched,
-                                  void* assign_ws, size_t assign_ws_bytes, float* y_dev, void* vmm_ws, size_t vmm_ws_bytes,
-                                  float* y_host, int flags, void* stream) {
-    if (!x_host_f16 || !x_dev_f16 || !y_dev || !y_host || !gsched) return GRINQH_ERR_NULL;
+                                  void* x_dev_f16, float* y_dev, void* vmm_ws, size_t vmm_ws_bytes, float* y_host,
+                                  int flags, void* stream) {
+    // every argument is checked before the first enqueue: on error nothing has been enqueued
+    if (!x_host_f16 || !x_dev_f16 || !y_dev || !y_host || !counts || !planes || !scales_f16 || !zeros_f16 || !vmm_ws)
+        return GRINQH_ERR_NULL;
     if (T < 1 || T > GRINQH_MAX_T || K <= 0 || N <= 0 || K % GQ_G || N % 32 || group != GQ_G || K > GQ_MAX_K)
         return GRINQH_ERR_SHAPE;
-    if (vmm_ws_bytes < grinqh_vmm_workspace_bytes(T, K, N)) return GRINQH_ERR_WORKSPACE;
+    if (((uintptr_t)x_dev_f16 | (uintptr_t)y_dev | (uintptr_t)planes | (uintptr_t)scales_f16 | (uintptr_t)zeros_f16 |
+         (uintptr_t)vmm_ws) & 15)
+        return GRINQH_ERR_ALIGN;
+    const size_t need = grinqh_vmm_workspace_bytes(T, K, N);
+    if (need == 0) return GRINQH_ERR_SHAPE;
+    if (vmm_ws_bytes < need) return GRINQH_ERR_WORKSPACE;
+    unsigned long long total = 0;
+    for (int w = 0; w < 9; ++w) total += counts[w];
+    if (total != (unsigned long long)K) return GRINQH_ERR_MIX;
     cudaStream_t st = (cudaStream_t)stream;
-    int rc = GRINQH_OK;
-    // Pinned (page-locked) host buffers are visible to the device under unified addressing: the assignment kernel
-    // then reads x straight from host memory (8-57 KB, once) and the VMM's second pass writes y straight into it —
-    // no copy nodes, no staging.  Pageable buffers (or GRINQH_FORCE_COPIES) go through cudaMemcpyAsync + staging.
-    auto device_view = [&](const void* host) -> void* {
-        if (flags & GRINQH_FORCE_COPIES) return nullptr;
+    // x: one small copy to the device (every CTA of the VMM reads all of x for its rank selection: that traffic
+    // belongs in L2, not on PCIe).  y: with a pinned (page-locked) host buffer the VMM's second pass writes the result
+    // straight into host memory — no copy node; a pageable buffer (or GRINQH_FORCE_COPIES) is staged through y_dev.
+    float* yv = nullptr;
+    if (!(flags & GRINQH_FORCE_COPIES)) {
         cudaPointerAttributes a;
-        if (cudaPointerGetAttributes(&a, host) != cudaSuccess) {
+        if (cudaPointerGetAttributes(&a, y_host) == cudaSuccess) {
+            if (a.type == cudaMemoryTypeHost && a.devicePointer && !((uintptr_t)a.devicePointer & 15))
+                yv = (float*)a.devicePointer;
+        } else {
             (void)cudaGetLastError();
-            return nullptr;
         }
-        return (a.type == cudaMemoryTypeHost && a.devicePointer && !((uintptr_t)a.devicePointer & 15)) ? a.devicePointer
-                                                                                                     : nullptr;
-    };
-    if (!(flags & GRINQH_REUSE_ASSIGNMENT)) {
-        const void* xv = device_view(x_host_f16);
-        if (!xv) {
-            if (cudaMemcpyAsync(x_dev_f16, x_host_f16, (size_t)T * K * 2, cudaMemcpyHostToDevice, st) != cudaSuccess)
-                return GRINQH_ERR_CUDA;
-            xv = x_dev_f16;
-        }
-        rc = grinqh_assign(xv, T, K, counts, bits, bits_union, rows, cnt_ge, grows, gcnt_ge, gsched, assign_ws,
-                           assign_ws_bytes, stream);
-        if (rc != GRINQH_OK) return rc;
     }
-    float* yv = (float*)device_view(y_host);
-    rc = grinqh_vmm(T, K, N, group, planes, scales_f16, zeros_f16, gsched, gcnt_ge, yv ? yv : y_dev, vmm_ws,
-                    vmm_ws_bytes, stream);
+    if (cudaMemcpyAsync(x_dev_f16, x_host_f16, (size_t)T * K * 2, cudaMemcpyHostToDevice, st) != cudaSuccess)
+        return GRINQH_ERR_CUDA;
+    const int rc = grinqh_vmm_rank(x_dev_f16, T, K, N, group, counts, planes, scales_f16, zeros_f16, yv ? yv : y_dev,
+                                   vmm_ws, vmm_ws_bytes, stream);
     if (rc != GRINQH_OK) return rc;
     if (!yv && cudaMemcpyAsync(y_host, y_dev, (size_t)T * N * 4, cudaMemcpyDeviceToHost, st) != cudaSuccess)
         return GRINQH_ERR_CUDA;

@@ -31,8 +31,7 @@ static int num_sms() {
     return cached[dev];
 }
 
-// Shape-only plan (the workspace size depends on it): one CTA per SM, as many split-K slices as fit; warps per CTA
-// such that a warp has about 24 rows or more (the per-warp fixed work is ~10 rows' worth of instructions).
+// Shape-only plan (the workspace size depends on it): one CTA per SM, as many split-K slices as fit.
 static inline VmmPlan vmm_plan(int T, int K, int N) {
     VmmPlan pl;
     pl.col_tiles = (N + TILE_COLS - 1) / TILE_COLS;
@@ -43,8 +42,7 @@ static inline VmmPlan vmm_plan(int T, int K, int N) {
     pl.Sx = sx;
     pl.vw = 8;
     if (T == 1) {
-        const int rows_per_cta = K / sx;  // upper bound: every row fetched
-        pl.vw = rows_per_cta >= 16 * 28 ? 16 : (rows_per_cta >= 8 * 28 || K > 16384) ? 8 : 4;
+        pl.vw = 16;  // measured: 16 warps win at every shape (4 and 8 leave the schedulers without enough warps)
         if (const char* f = getenv("GRINQH_VW")) {  // measurement override
             const int v = atoi(f);
             if (v == 4 || v == 8 || v == 16) pl.vw = v;

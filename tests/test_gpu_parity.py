@@ -228,24 +228,25 @@ def test_decode_host_entry(gq):
     planes, s, z = oracle.pack(W)
     y_ref = oracle.vmm(x, planes, s, z, oracle.assign(x, counts)["bits"])
     w = gq.grinqh_pack(_dev(W))
-    a = gq.Assignment(1, K)
     xh = torch.from_numpy(x).pin_memory()
     yh = torch.empty((1, N), dtype=torch.float32).pin_memory()
     xd = torch.empty((1, K), dtype=torch.float16, device="cuda")
     yd = torch.empty((1, N), dtype=torch.float32, device="cuda")
     ws = gq.grinqh_vmm_workspace(1, K, N)
-    gq.grinqh_decode_host(xh, counts, w, a, xd, yd, ws, yh)           # pinned: kernels access host memory directly
+    gq.grinqh_decode_host(xh, counts, w, xd, yd, ws, yh)           # pinned y: the kernel writes host memory directly
     torch.cuda.synchronize()
     assert rel_l2(yh.numpy(), y_ref) <= TOL
     y_direct = yh.numpy().copy()
     yh.zero_()
-    gq.grinqh_decode_host(xh, counts, w, a, xd, yd, ws, yh, force_copies=True)   # staged with cudaMemcpyAsync
+    gq.grinqh_decode_host(xh, counts, w, xd, yd, ws, yh, force_copies=True)   # staged with cudaMemcpyAsync
     torch.cuda.synchronize()
     assert np.array_equal(yh.numpy(), y_direct)
     xp, yp = torch.from_numpy(x.copy()), torch.zeros((1, N), dtype=torch.float32)   # pageable host buffers
-    gq.grinqh_decode_host(xp, counts, w, a, xd, yd, ws, yp)
+    gq.grinqh_decode_host(xp, counts, w, xd, yd, ws, yp)
     torch.cuda.synchronize()
     assert np.array_equal(yp.numpy(), y_direct)
+    with pytest.raises(gq.GrinqhError):                             # a bad mix is rejected before anything is enqueued
+        gq.grinqh_decode_host(xh, [K, 1, 0, 0, 0, 0, 0, 0, 0], w, xd, yd, ws, yh)
 
 
 def test_fused_second_pass_matches_two_launches_and_workspace_is_reusable(gq):
