@@ -31,6 +31,30 @@ def test_library_exports_every_declared_symbol(lib):
     assert set(binding.EXPORTS) == declared
 
 
+def test_mix_to_counts_closed_forms(lib):
+    """The product's own copy pinned directly (not through the oracle's): the config mixes are multiples of 1/32 and the
+    config K multiples of 256, so counts = frac * K exactly; an arbitrary mix always sums to K, is monotone in the
+    cumulative shares, and is within one row of frac * K per width boundary."""
+    lib.grinqh_mix_to_counts.argtypes = [C.c_int, C.c_void_p, C.c_void_p]
+    for K in (256, 4096, 12288, 14336, 8192, 28672):
+        for name, frac in synth.MIXES.items():
+            f = (C.c_double * 9)(*frac)
+            c = (C.c_uint32 * 9)()
+            assert lib.grinqh_mix_to_counts(K, f, c) == 0
+            assert list(c) == [int(round(p * K)) for p in frac] and all(abs(p * K - round(p * K)) < 1e-9 for p in frac)
+    rng = np.random.default_rng(1)
+    for _ in range(50):
+        K = 128 * int(rng.integers(1, 257))
+        frac = rng.dirichlet(np.ones(9))
+        f = (C.c_double * 9)(*frac)
+        c = (C.c_uint32 * 9)()
+        assert lib.grinqh_mix_to_counts(K, f, c) == 0
+        assert sum(c) == K
+        cum_c = np.cumsum(list(c)[::-1])[:-1]              # rows with width >= w, w = 8..1
+        cum_f = np.cumsum(frac[::-1])[:-1] * K
+        assert np.all(np.abs(cum_c - cum_f) <= 0.5 + 1e-6)  # C_w = floor(F_w K + 1/2)
+
+
 def test_mix_to_counts_matches_oracle_and_rejects(lib):
     lib.grinqh_mix_to_counts.argtypes = [C.c_int, C.c_void_p, C.c_void_p]
     rng = np.random.default_rng(0)
@@ -73,6 +97,16 @@ def test_argument_validation_without_gpu(lib):
     assert lib.grinqh_vmm_workspace_bytes(1, 32768, 4096) > 0 and lib.grinqh_vmm_workspace_bytes(1, 32768 + 128, 4096) == 0
     lib.grinqh_vmm.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int] + [vp] * 5 + [vp, vp, C.c_size_t, vp]
     assert lib.grinqh_vmm(1, 128, 32, 128, 16, 16, 16, 16, 16, 16, 16, 0, None) == -5  # workspace
+    lib.grinqh_vmm_rank.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.c_int, vp] + [vp] * 3 + [vp, vp, C.c_size_t, vp]
+    big = 1 << 30
+    assert lib.grinqh_vmm_rank(16, 1, 128, 32, 128, counts, 16, 16, 16, 16, 16, big, None) == -4   # sum(counts) != K
+    assert lib.grinqh_vmm_rank(16, 1, 128, 32, 128, None, 16, 16, 16, 16, 16, big, None) == -1     # NULL counts
+    lib.grinqh_decode_host.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.c_int, vp] + [vp] * 3 + [vp, vp, vp,
+                                                                                                  C.c_size_t, vp, C.c_int, vp]
+    # every argument is validated before anything is enqueued (no GPU is touched here)
+    assert lib.grinqh_decode_host(16, 1, 128, 32, 128, counts, 16, 16, 16, 16, 16, 16, big, 16, 0, None) == -4
+    assert lib.grinqh_decode_host(16, 1, 128, 32, 128, counts, 16, 16, 16, 16, 16, 16, 0, 16, 0, None) == -5
+    assert lib.grinqh_decode_host(16, 1, 128, 40, 128, counts, 16, 16, 16, 16, 16, 16, big, 16, 0, None) == -2
 
 
 def test_gather_network_on_host(tmp_path):
