@@ -193,3 +193,56 @@ def dequant(planes, scales, zeros, b: int, G: int = 128) -> np.ndarray:
     w = np.zeros((K, N), dtype=np.float64)
     lib().orc_dequant(_p(planes), _p(_u16(scales)), _p(_u16(zeros)), K, N, G, int(b), _p(w))
     return w
+
+
+# ---- 2-bit-segment store, bmax in {4, 6, 8}
+def code2_prime(q: int, b: int, bmax: int) -> int:
+    return int(lib().orc_code2_prime(int(q), int(b), int(bmax)))
+
+
+def pack2(W, bmax: int, G: int = 128):
+    """W [K, N] fp16 -> segs [bmax/2, K, N/16] uint32, scales / zeros [K/G, N] fp16."""
+    W = np.ascontiguousarray(W)
+    K, N = W.shape
+    segs = np.zeros((bmax // 2, K, N // 16), dtype=np.uint32)
+    s = np.zeros((K // G, N), dtype=np.float16)
+    z = np.zeros((K // G, N), dtype=np.float16)
+    rc = lib().orc_pack2(_p(_u16(W)), K, N, G, int(bmax), _p(segs), _p(s.view(np.uint16)), _p(z.view(np.uint16)))
+    if rc:
+        raise ValueError(f"orc_pack2 failed: {rc}")
+    return segs, s, z
+
+
+def codes2(segs, bmax: int) -> np.ndarray:
+    _, K, words = segs.shape
+    q = np.zeros((K, words * 16), dtype=np.uint8)
+    lib().orc_codes2(_p(np.ascontiguousarray(segs)), K, words * 16, int(bmax), _p(q))
+    return q
+
+
+def vmm2(x, segs, scales, zeros, bits, bmax: int, G: int = 128, cols=None) -> np.ndarray:
+    x = np.ascontiguousarray(x)
+    T, K = x.shape
+    N = segs.shape[2] * 16
+    bits = np.ascontiguousarray(bits, dtype=np.uint8)
+    if cols is None:
+        ncols, cp = N, None
+    else:
+        cols = np.ascontiguousarray(cols, dtype=np.int32)
+        ncols, cp = len(cols), _p(cols)
+    y = np.zeros((T, ncols), dtype=np.float64)
+    rc = lib().orc_vmm2_cols(_p(_u16(x)), T, K, N, G, int(bmax), _p(np.ascontiguousarray(segs)),
+                             _p(_u16(scales)), _p(_u16(zeros)), _p(bits), cp, ncols, _p(y))
+    if rc:
+        raise ValueError(f"orc_vmm2_cols failed: {rc}")
+    return y
+
+
+def dequant2(segs, scales, zeros, bmax: int, b: int, G: int = 128) -> np.ndarray:
+    _, K, words = segs.shape
+    w = np.zeros((K, words * 16), dtype=np.float64)
+    rc = lib().orc_dequant2(_p(np.ascontiguousarray(segs)), _p(_u16(scales)), _p(_u16(zeros)), K, words * 16, G,
+                            int(bmax), int(b), _p(w))
+    if rc:
+        raise ValueError(f"orc_dequant2 failed: {rc}")
+    return w

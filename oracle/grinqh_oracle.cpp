@@ -108,6 +108,31 @@ inline int code_from_planes(const uint32_t* planes, int K, int N, int k, int n, 
     return q;
 }
 
+
+// ---- the paper's own granularity — 2-bit significance segments, b in {0, 2, .., bmax},
+//      bmax in {4, 6, 8} (PAPER.md:79-81 "decomposed into discrete 2-bit segments", :95, :262, :440-444).
+// Layout of this build, defined here by formula (reading #10b): segs[sigma][k][n >> 4], sigma = 0 is the most
+// significant pair; column n's pair sits at bits 2 (n & 15) + 1 (code bit bmax - 1 - 2 sigma) and 2 (n & 15)
+// (code bit bmax - 2 - 2 sigma) of the word: sixteen 2-bit chunks per uint32.
+inline int phi2_of(int b, int bmax) {  // phi = 2^(bmax - b - 1); reading #5: 0 at b = bmax
+    return (b >= 1 && b < bmax) ? (1 << (bmax - b - 1)) : 0;
+}
+inline int code2_prime(int q, int b, int bmax) {  // q_b 2^(bmax - b) + phi, q_b = the top b bits of the bmax-bit code
+    if (b <= 0) return 0;
+    int qb = q >> (bmax - b);
+    return (qb << (bmax - b)) | phi2_of(b, bmax);
+}
+inline int code_from_segs(const uint32_t* segs, int K, int N, int k, int n, int b, int bmax) {
+    const size_t words = (size_t)N / 16;
+    const size_t seg_stride = (size_t)K * words;
+    int q = 0;
+    for (int sg = 0; sg < b / 2; ++sg) {  // only the first b / 2 segments are read (nested property)
+        uint32_t w = segs[(size_t)sg * seg_stride + (size_t)k * words + (size_t)(n >> 4)];
+        q |= (int)((w >> (2 * (n & 15))) & 3u) << (bmax - 2 - 2 * sg);
+    }
+    return q;
+}
+
 }  // namespace
 
 extern "C" {
@@ -409,6 +434,106 @@ int orc_dequant(const uint32_t* planes, const uint16_t* scales, const uint16_t* 
             double s = (double)half_to_float(scales[(size_t)(k / G) * N + n]);
             double z = (double)half_to_float(zeros[(size_t)(k / G) * N + n]);
             w_hat[(size_t)k * N + n] = s * (double)code_prime(q, b) + z;
+        }
+    return 0;
+}
+
+// ---- 8f2 entry points (2-bit segments, bmax in {4, 6, 8})
+int orc_code2_prime(int q, int b, int bmax) { return code2_prime(q, b, bmax); }
+
+// Quantiser of orc_pack with 2^bmax - 1 steps (reading #8), codes split into bmax / 2 segment arrays.
+int orc_pack2(const uint16_t* W, int K, int N, int G, int bmax, uint32_t* segs, uint16_t* scales, uint16_t* zeros) {
+    if (K % G || N % 16 || (bmax != 4 && bmax != 6 && bmax != 8)) return -2;
+    const size_t words = (size_t)N / 16;
+    const size_t seg_stride = (size_t)K * words;
+    const float qmax = (float)((1 << bmax) - 1);
+    std::memset(segs, 0, sizeof(uint32_t) * (bmax / 2) * seg_stride);
+    for (int g = 0; g < K / G; ++g) {
+        for (int n = 0; n < N; ++n) {
+            float lo = half_to_float(W[(size_t)(g * G) * N + n]);
+            float hi = lo;
+            uint16_t lo_bits = W[(size_t)(g * G) * N + n];
+            for (int i = 1; i < G; ++i) {
+                uint16_t hb = W[(size_t)(g * G + i) * N + n];
+                float v = half_to_float(hb);
+                if (v < lo) {
+                    lo = v;
+                    lo_bits = hb;
+                }
+                if (v > hi) hi = v;
+            }
+            if (lo == 0.0f) lo_bits = 0;
+            volatile float range = hi - lo;
+            volatile float s32 = range / qmax;
+            uint16_t s_bits = float_to_half(s32);
+            float s = half_to_float(s_bits);
+            float z = half_to_float(lo_bits);
+            scales[(size_t)g * N + n] = s_bits;
+            zeros[(size_t)g * N + n] = lo_bits;
+            for (int i = 0; i < G; ++i) {
+                int k = g * G + i;
+                int q = 0;
+                if (s != 0.0f) {
+                    volatile float d = half_to_float(W[(size_t)k * N + n]) - z;
+                    volatile float t = d / s;
+                    float r = std::nearbyintf(t);
+                    if (r < 0.0f) r = 0.0f;
+                    if (r > qmax) r = qmax;
+                    q = (int)r;
+                }
+                for (int sg = 0; sg < bmax / 2; ++sg) {
+                    uint32_t pair = (uint32_t)(q >> (bmax - 2 - 2 * sg)) & 3u;
+                    segs[(size_t)sg * seg_stride + (size_t)k * words + (size_t)(n >> 4)] |= pair << (2 * (n & 15));
+                }
+            }
+        }
+    }
+    return 0;
+}
+
+int orc_codes2(const uint32_t* segs, int K, int N, int bmax, uint8_t* q) {
+    for (int k = 0; k < K; ++k)
+        for (int n = 0; n < N; ++n) q[(size_t)k * N + n] = (uint8_t)code_from_segs(segs, K, N, k, n, bmax, bmax);
+    return 0;
+}
+
+// y[t][n] = sum_{k : b_tk > 0} x_tk ( s_gn code2'(q_kn, b_tk) + z_gn )  — PAPER.md:85 with the store's own bmax
+int orc_vmm2_cols(const uint16_t* x, int T, int K, int N, int G, int bmax, const uint32_t* segs, const uint16_t* scales,
+                  const uint16_t* zeros, const uint8_t* bits, const int32_t* cols, int ncols, double* y) {
+    for (size_t i = 0; i < (size_t)T * K; ++i)
+        if (bits[i] > bmax || (bits[i] & 1)) return -2;  // widths are 0, 2, .., bmax
+    for (int t = 0; t < T; ++t) {
+        for (int c = 0; c < ncols; ++c) {
+            int n = cols ? cols[c] : c;
+            double acc = 0.0;
+            for (int k = 0; k < K; ++k) {
+                int b = bits[(size_t)t * K + k];
+                if (b == 0) continue;
+                int g = k / G;
+                int q = code_from_segs(segs, K, N, k, n, b, bmax);
+                double s = (double)half_to_float(scales[(size_t)g * N + n]);
+                double z = (double)half_to_float(zeros[(size_t)g * N + n]);
+                acc += (double)half_to_float(x[(size_t)t * K + k]) * (s * (double)code2_prime(q, b, bmax) + z);
+            }
+            y[(size_t)t * ncols + c] = acc;
+        }
+    }
+    return 0;
+}
+
+int orc_dequant2(const uint32_t* segs, const uint16_t* scales, const uint16_t* zeros, int K, int N, int G, int bmax,
+                 int b, double* w_hat) {
+    if (b > bmax || (b & 1)) return -2;
+    for (int k = 0; k < K; ++k)
+        for (int n = 0; n < N; ++n) {
+            if (b == 0) {
+                w_hat[(size_t)k * N + n] = 0.0;
+                continue;
+            }
+            int q = code_from_segs(segs, K, N, k, n, b, bmax);
+            double s = (double)half_to_float(scales[(size_t)(k / G) * N + n]);
+            double z = (double)half_to_float(zeros[(size_t)(k / G) * N + n]);
+            w_hat[(size_t)k * N + n] = s * (double)code2_prime(q, b, bmax) + z;
         }
     return 0;
 }
