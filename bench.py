@@ -55,6 +55,7 @@ def _args():
     ap.add_argument("--prefill", action="store_true", help="f3 (part): grinqh_unpack + dense library GEMM timings")
     ap.add_argument("--decode-step", action="store_true", help="config 4: 32-layer decode step in one CUDA graph")
     ap.add_argument("--no-split", action="store_true", help="skip the one-launch-per-projection variant")
+    ap.add_argument("--seg2", action="store_true", help="f2: 2-bit-segment store against the 1-bit plane store (A/B)")
     return ap.parse_args()
 
 
@@ -665,9 +666,72 @@ def run_prefill(args):
         del W, w, out, X
 
 
+# ------------------------------------------------------------------------------------------ f2: 2-bit segments A/B
+def run_seg2(args):
+    """SURVEY.md 8f2 / PAPER.md:79-81, :442: the same weights in the paper's 2-bit-segment store (b_max = 8) and in the
+    1-bit plane store, rank assignment inside the launch, per mix.  One JSON line per case, prefixed "SEG2 "."""
+    import math
+
+    import torch
+
+    from paper_2606_23419_b200 import binding as gq
+    from paper_2606_23419_b200 import synth
+
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    peak, _ = _peaks()
+    gen = torch.Generator(device=dev)
+    gen.manual_seed(args.seed)
+    stream = torch.cuda.Stream(device=dev)
+
+    def time_graph(fn, n_inner, reps=20):
+        with torch.cuda.stream(stream):
+            fn()
+            stream.synchronize()
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g, stream=stream):
+                fn()
+            for _ in range(3):
+                g.replay()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            stream.synchronize()
+            a.record(stream)
+            for _ in range(reps):
+                g.replay()
+            b.record(stream)
+            stream.synchronize()
+        return a.elapsed_time(b) * 1e3 / (reps * n_inner)
+
+    for K, N in [(4096, 28672), (8192, 28672), (14336, 4096)]:
+        copies = int(math.ceil(300e6 / (K * N))) + 1          # > 2 x L2 of 8-bit codes, rotated
+        planes, segs = [], []
+        for c in range(copies):
+            W = (torch.randn((K, N), generator=gen, device=dev, dtype=torch.float32) * 0.02).to(torch.float16)
+            planes.append(gq.grinqh_pack(W))
+            segs.append(gq.grinqh_pack_seg2(W, 8))
+            del W
+        ws = gq.grinqh_vmm_workspace(1, K, N, dev)
+        x = torch.from_numpy(synth.make_x(1, K, args.seed + 7, "normal")).to(dev)
+        y = torch.empty((1, N), dtype=torch.float32, device=dev)
+        for mix in ["2", "3", "4", "5", "8"]:
+            counts = gq.grinqh_mix_to_counts(K, synth.MIXES[mix])
+            bits = sum(w * c for w, c in enumerate(counts))
+            ab = alg_bytes(K, N, 1, bits)
+            us_p = time_graph(lambda: [gq.grinqh_vmm_rank(x, counts, w, y, ws) for w in planes], copies)
+            us_s = time_graph(lambda: [gq.grinqh_vmm_rank_seg2(x, counts, w, y, ws) for w in segs], copies)
+            print("SEG2 " + json.dumps({"K": K, "N": N, "mix": mix, "avg_bits": bits / K, "alg_MB": ab / 1e6,
+                                        "us_planes": us_p, "us_seg2": us_s, "seg2_over_planes": us_s / us_p,
+                                        "frac_planes": ab / us_p / 1e3 / peak, "frac_seg2": ab / us_s / 1e3 / peak}),
+                  flush=True)
+        del planes, segs
+        torch.cuda.empty_cache()
+
+
 def main():
     args = _args()
-    if args.prefill:
+    if args.seg2:
+        run_seg2(args)
+    elif args.prefill:
         run_prefill(args)
     elif args.decode_step:
         run_decode_step(args)

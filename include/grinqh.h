@@ -202,6 +202,24 @@ int grinqh_vmm_rank(const void* x_f16, int T, int K, int N, int group, const uin
                     float* y, void* workspace, size_t workspace_bytes, void* stream);
 
 /*
+ * The paper's own storage granularity ("decomposed into discrete 2-bit segments",
+ * :95 b_max in {4, 6, 8}, :442 sixteen 2-bit chunks per uint32): b_max-bit asymmetric group codes (the quantiser of
+ * grinqh_pack with 2^b_max - 1 steps) split into b_max / 2 two-bit significance segments.
+ *   segs  dev  [b_max/2][K][N/16] uint32: segment 0 is the most significant pair; column n's pair sits at bits
+ *              2 (n & 15) + 1 and 2 (n & 15) of word n >> 4.
+ * grinqh_pack_seg2: offline, once per weight (scales / zeros as in grinqh_pack).
+ * grinqh_vmm_rank_seg2: grinqh_vmm_rank over that store: widths in {0, 2, .., b_max} (counts[w] must be 0 for odd w
+ * and for w > b_max: GRINQH_ERR_MIX), a row of width b fetches its first b / 2 segments, reconstruction
+ * w_hat = s * (q_b * 2^(b_max - b) + 2^(b_max - b - 1)) + z (no bias at b = b_max).  One token (T = 1),
+ * N % 128 == 0 (GRINQH_ERR_SHAPE otherwise); workspace as for grinqh_vmm.
+ */
+int grinqh_pack_seg2(const void* W_f16, int K, int N, int group, int bmax,
+                     uint32_t* segs, void* scales_f16, void* zeros_f16, void* stream);
+int grinqh_vmm_rank_seg2(const void* x_f16, int T, int K, int N, int group, int bmax, const uint32_t counts[9],
+                         const uint32_t* segs, const void* scales_f16, const void* zeros_f16,
+                         float* y, void* workspace, size_t workspace_bytes, void* stream);
+
+/*
  * Host-buffer decode call (the end-to-end entry): x comes from HOST memory, the rank assignment and the VMM run in
  * one launch (grinqh_vmm_rank), y ends in HOST memory, all enqueued on `stream`.  x is staged with one
  * cudaMemcpyAsync (every CTA reads all of x for its rank selection).  With a pinned (page-locked) y_host the VMM's

@@ -54,6 +54,10 @@ _lib.grinqh_vmm_thresholds.restype = _i
 _lib.grinqh_vmm_thresholds.argtypes = [_vp, _i, _i, _i, _i, _vp, _vp, _vp, _vp, _vp, _vp, _sz, _vp]
 _lib.grinqh_vmm_rank.restype = _i
 _lib.grinqh_vmm_rank.argtypes = [_vp, _i, _i, _i, _i, _vp, _vp, _vp, _vp, _vp, _vp, _sz, _vp]
+_lib.grinqh_pack_seg2.restype = _i
+_lib.grinqh_pack_seg2.argtypes = [_vp, _i, _i, _i, _i, _vp, _vp, _vp, _vp]
+_lib.grinqh_vmm_rank_seg2.restype = _i
+_lib.grinqh_vmm_rank_seg2.argtypes = [_vp, _i, _i, _i, _i, _i, _vp, _vp, _vp, _vp, _vp, _vp, _sz, _vp]
 _lib.grinqh_vmm_main.restype = _i
 _lib.grinqh_vmm_main.argtypes = _VMM_COMMON + [_vp, _sz, _vp]
 _lib.grinqh_vmm_reduce.restype = _i
@@ -65,7 +69,7 @@ EXPORTS = ("grinqh_status_string", "grinqh_version", "grinqh_mix_to_counts", "gr
            "grinqh_assign_workspace_bytes", "grinqh_assign", "grinqh_assign_thresholds",
            "grinqh_calibrate_thresholds", "grinqh_vmm_workspace_bytes",
            "grinqh_vmm_workspace_init", "grinqh_vmm", "grinqh_vmm_thresholds", "grinqh_vmm_rank",
-           "grinqh_vmm_main", "grinqh_vmm_reduce", "grinqh_decode_host")
+           "grinqh_vmm_main", "grinqh_vmm_reduce", "grinqh_decode_host", "grinqh_pack_seg2", "grinqh_vmm_rank_seg2")
 
 
 class GrinqhError(RuntimeError):
@@ -244,6 +248,38 @@ def grinqh_vmm_rank(x: torch.Tensor, counts, w: Packed, y: torch.Tensor | None =
     _check(_lib.grinqh_vmm_rank(_dev(x, torch.float16, "x"), T, K, w.N, GROUP, _counts(counts), w.planes.data_ptr(),
                                 w.scales.data_ptr(), w.zeros.data_ptr(), _dev(y, torch.float32, "y"),
                                 workspace.data_ptr(), nbytes, _stream(stream)), "grinqh_vmm_rank")
+    return y
+
+
+class PackedSeg2:
+    """Device-resident 2-bit-segment store: segs [bmax/2, K, N/16] int32 (bit patterns), scales/zeros [K/128, N] fp16."""
+
+    def __init__(self, K: int, N: int, bmax: int, device="cuda"):
+        self.K, self.N, self.bmax = K, N, bmax
+        self.segs = torch.empty((bmax // 2, K, N // 16), dtype=torch.int32, device=device)
+        self.scales = torch.empty((K // GROUP, N), dtype=torch.float16, device=device)
+        self.zeros = torch.empty((K // GROUP, N), dtype=torch.float16, device=device)
+
+
+def grinqh_pack_seg2(W: torch.Tensor, bmax: int, out: PackedSeg2 | None = None, stream=None) -> PackedSeg2:
+    K, N = W.shape
+    out = out or PackedSeg2(K, N, bmax, W.device)
+    _check(_lib.grinqh_pack_seg2(_dev(W, torch.float16, "W"), K, N, GROUP, int(bmax), out.segs.data_ptr(),
+                                 out.scales.data_ptr(), out.zeros.data_ptr(), _stream(stream)), "grinqh_pack_seg2")
+    return out
+
+
+def grinqh_vmm_rank_seg2(x: torch.Tensor, counts, w: PackedSeg2, y: torch.Tensor | None = None,
+                         workspace: torch.Tensor | None = None, stream=None) -> torch.Tensor:
+    """y [1, N] = x . W over the 2-bit-segment store, rank assignment inside the launch (widths 0, 2, .., bmax)."""
+    T, K = x.shape
+    if y is None:
+        y = torch.empty((T, w.N), dtype=torch.float32, device=x.device)
+    workspace, nbytes = _ws(T, K, w.N, workspace, x.device)
+    _check(_lib.grinqh_vmm_rank_seg2(_dev(x, torch.float16, "x"), T, K, w.N, GROUP, w.bmax, _counts(counts),
+                                     w.segs.data_ptr(), w.scales.data_ptr(), w.zeros.data_ptr(),
+                                     _dev(y, torch.float32, "y"), workspace.data_ptr(), nbytes, _stream(stream)),
+           "grinqh_vmm_rank_seg2")
     return y
 
 

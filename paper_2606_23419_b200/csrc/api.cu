@@ -85,6 +85,17 @@ extern "C" int grinqh_calibrate_thresholds(const void* x_host_f16, int S, int K,
     return GRINQH_OK;
 }
 
+namespace gq {
+// x from pinned host memory to its device staging buffer: ONE small CTA reads the few KB over PCIe (host-mapped
+// access), so that the 148 CTAs of the VMM read x from L2.  A kernel, not a copy node: it chains to its neighbours with
+// programmatic dependent launch like every other launch of the step.
+__global__ void __launch_bounds__(512) stage_x_kernel(const uint4* __restrict__ src, uint4* __restrict__ dst, int n16) {
+    pdl_launch_dependents();
+    pdl_wait();
+    for (int i = threadIdx.x; i < n16; i += 512) dst[i] = src[i];
+}
+}  // namespace gq
+
 extern "C" int grinqh_decode_host(const void* x_host_f16, int T, int K, int N, int group, const uint32_t counts[9],
                                   const uint32_t* planes, const void* scales_f16, const void* zeros_f16,
                                   void* x_dev_f16, float* y_dev, void* vmm_ws, size_t vmm_ws_bytes, float* y_host,
@@ -105,7 +116,7 @@ extern "C" int grinqh_decode_host(const void* x_host_f16, int T, int K, int N, i
     if (total != (unsigned long long)K) return GRINQH_ERR_MIX;
     cudaStream_t st = (cudaStream_t)stream;
     // x: one small copy to the device (every CTA of the VMM reads all of x for its rank selection: that traffic
-    // belongs in L2, not on PCIe).  y: with a pinned (page-locked) host buffer the VMM's second pass writes the result
+    // belongs in L2, not on PCIe) — by a one-CTA kernel reading the pinned buffer directly, else by cudaMemcpyAsync.  y: with a pinned (page-locked) host buffer the VMM's second pass writes the result
     // straight into host memory — no copy node; a pageable buffer (or GRINQH_FORCE_COPIES) is staged through y_dev.
     float* yv = nullptr;
     if (!(flags & GRINQH_FORCE_COPIES)) {
@@ -117,8 +128,22 @@ extern "C" int grinqh_decode_host(const void* x_host_f16, int T, int K, int N, i
             (void)cudaGetLastError();
         }
     }
-    if (cudaMemcpyAsync(x_dev_f16, x_host_f16, (size_t)T * K * 2, cudaMemcpyHostToDevice, st) != cudaSuccess)
+    const void* xv = nullptr;  // device view of a pinned x_host
+    if (!(flags & GRINQH_FORCE_COPIES)) {
+        cudaPointerAttributes a;
+        if (cudaPointerGetAttributes(&a, x_host_f16) == cudaSuccess) {
+            if (a.type == cudaMemoryTypeHost && a.devicePointer && !((uintptr_t)a.devicePointer & 15)) xv = a.devicePointer;
+        } else {
+            (void)cudaGetLastError();
+        }
+    }
+    if (xv) {
+        if (gq::launch_pdl(gq::stage_x_kernel, dim3(1), dim3(512), 0, st, (const uint4*)xv, (uint4*)x_dev_f16,
+                           T * K / 8) != cudaSuccess)
+            return GRINQH_ERR_CUDA;
+    } else if (cudaMemcpyAsync(x_dev_f16, x_host_f16, (size_t)T * K * 2, cudaMemcpyHostToDevice, st) != cudaSuccess) {
         return GRINQH_ERR_CUDA;
+    }
     const int rc = grinqh_vmm_rank(x_dev_f16, T, K, N, group, counts, planes, scales_f16, zeros_f16, yv ? yv : y_dev,
                                    vmm_ws, vmm_ws_bytes, stream);
     if (rc != GRINQH_OK) return rc;

@@ -71,4 +71,23 @@ GQ_HD void gather(const uint32_t (&W)[8], uint32_t (&V)[8]) {
     tstep<4, (B <= 4)>(V[3], V[7]);
 }
 
+// ---- 2-bit-segment store.  a[sg], sg < NS: the segment words of one 16-column
+// half (column c's pair at bits 2c + 1, 2c; segment 0 = the most significant pair).  X[j], j = 0..3: byte i = the code
+// of column 4 i + j, left-aligned in the byte (segment sg at bits 7 - 2 sg, 6 - 2 sg), missing segments zero.  Two
+// stages of a 4 x 4 transpose of 2-bit elements: the first butterfly stage of the 1-bit store is already in the layout.
+template <int NS>
+GQ_HD void gather_seg2(const uint32_t (&a)[4], uint32_t (&X)[4]) {
+    static_assert(NS >= 1 && NS <= 4, "1 to 4 segments");
+    constexpr uint32_t M2 = 0x33333333u, M4 = 0x0F0F0F0Fu;
+    // nibble j of pe / po = (a0 element << 2) | a1 element of columns 2 j / 2 j + 1; qe / qo the same of a2, a3
+    const uint32_t pe = (NS >= 2) ? (((a[0] << 2) & ~M2) | (a[1] & M2)) : ((a[0] << 2) & ~M2);
+    const uint32_t po = (NS >= 2) ? ((a[0] & ~M2) | ((a[1] >> 2) & M2)) : (a[0] & ~M2);
+    const uint32_t qe = (NS >= 4) ? (((a[2] << 2) & ~M2) | (a[3] & M2)) : (NS == 3) ? ((a[2] << 2) & ~M2) : 0u;
+    const uint32_t qo = (NS >= 4) ? ((a[2] & ~M2) | ((a[3] >> 2) & M2)) : (NS == 3) ? (a[2] & ~M2) : 0u;
+    X[0] = ((pe & M4) << 4) | (qe & M4);
+    X[2] = (pe & ~M4) | ((qe >> 4) & M4);
+    X[1] = ((po & M4) << 4) | (qo & M4);
+    X[3] = (po & ~M4) | ((qo >> 4) & M4);
+}
+
 }  // namespace gq

@@ -39,6 +39,32 @@ static inline VmmPlan vmm_plan(int T, int K, int N) {
     const int cap = K / 64 > 0 ? K / 64 : 1;
     if (sx > cap) sx = cap;
     if (sx < 1) sx = 1;
+    // Among the few largest split factors take the one sharing the largest factor with the number of groups: the CTAs'
+    // slot ranges then line up with group boundaries more often (fewer warps straddle two groups and pay two sets of
+    // scale/zero chunks).  Measured (profiles/r02_kernels.md): 4096 x 4096 36 slices 13.1 us against 14.6 us with 37;
+    // 14336 x 4096 35 slices 19.1 us against 20.7 us with 37.
+    {
+        auto gcd = [](int a, int b) {
+            while (b) {
+                const int t = a % b;
+                a = b;
+                b = t;
+            }
+            return a;
+        };
+        const int groups = K / GQ_G;
+        int best = sx, best_g = gcd(groups, sx);
+        for (int c = sx - 1; c >= 1 && c * 100 >= sx * 94; --c)
+            if (gcd(groups, c) > best_g) {
+                best = c;
+                best_g = gcd(groups, c);
+            }
+        sx = best;
+    }
+    if (const char* f = getenv("GRINQH_SX")) {  // measurement override
+        const int v = atoi(f);
+        if (v >= 1 && v <= sx) sx = v;
+    }
     pl.Sx = sx;
     pl.vw = 8;
     if (T == 1) {
@@ -132,7 +158,7 @@ extern "C" int grinqh_vmm(int T, int K, int N, int group, const uint32_t* planes
     const int rc = gq::check_vmm_ptrs(T, K, N, group, planes, scales_f16, zeros_f16, gsched, gcnt_ge, workspace,
                                       workspace_bytes);
     if (rc != GRINQH_OK) return rc;
-    gq::VmmArgs a{T, K, N, 1, gq::MODE_SCHED, planes, scales_f16, zeros_f16, gsched, gcnt_ge, nullptr, gq::CutParams{},
+    gq::VmmArgs a{T, K, N, 1, gq::MODE_SCHED, 8, planes, scales_f16, zeros_f16, gsched, gcnt_ge, nullptr, gq::CutParams{},
                   workspace, y, (cudaStream_t)stream};
     return gq::launch_vmm(a);
 }
@@ -143,7 +169,7 @@ extern "C" int grinqh_vmm_main(int T, int K, int N, int group, const uint32_t* p
     const int rc = gq::check_vmm_ptrs(T, K, N, group, planes, scales_f16, zeros_f16, gsched, gcnt_ge, workspace,
                                       workspace_bytes);
     if (rc != GRINQH_OK) return rc;
-    gq::VmmArgs a{T, K, N, 0, gq::MODE_SCHED, planes, scales_f16, zeros_f16, gsched, gcnt_ge, nullptr, gq::CutParams{},
+    gq::VmmArgs a{T, K, N, 0, gq::MODE_SCHED, 8, planes, scales_f16, zeros_f16, gsched, gcnt_ge, nullptr, gq::CutParams{},
                   workspace, nullptr, (cudaStream_t)stream};
     return gq::launch_vmm(a);
 }
@@ -175,7 +201,7 @@ extern "C" int grinqh_vmm_thresholds(const void* x_f16, int T, int K, int N, int
     if (rc != GRINQH_OK) return rc;
     for (int w = 1; w <= 8; ++w)
         if (theta[w] > 0x8000 || (w > 1 && theta[w] < theta[w - 1])) return GRINQH_ERR_MIX;
-    gq::VmmArgs a{T, K, N, 1, gq::MODE_THR, planes, scales_f16, zeros_f16, nullptr, nullptr, (const uint16_t*)x_f16,
+    gq::VmmArgs a{T, K, N, 1, gq::MODE_THR, 8, planes, scales_f16, zeros_f16, nullptr, nullptr, (const uint16_t*)x_f16,
                   gq::cuts_from_thetas(theta), workspace, y, (cudaStream_t)stream};
     return gq::launch_vmm(a);
 }
@@ -193,7 +219,30 @@ extern "C" int grinqh_vmm_rank(const void* x_f16, int T, int K, int N, int group
     unsigned long long total = 0;
     for (int w = 0; w < 9; ++w) total += counts[w];
     if (total != (unsigned long long)K) return GRINQH_ERR_MIX;
-    gq::VmmArgs a{T, K, N, 1, gq::MODE_RANK, planes, scales_f16, zeros_f16, nullptr, nullptr, (const uint16_t*)x_f16,
+    gq::VmmArgs a{T, K, N, 1, gq::MODE_RANK, 8, planes, scales_f16, zeros_f16, nullptr, nullptr, (const uint16_t*)x_f16,
                   gq::cuts_from_counts(counts), workspace, y, (cudaStream_t)stream};
     return gq::launch_vmm(a);
+}
+
+// the same launch over the paper's own store — b_max-bit codes in 2-bit significance segments
+// (grinqh_pack_seg2), widths in {0, 2, .., b_max}.  One token, N % 128 == 0.
+extern "C" int grinqh_vmm_rank_seg2(const void* x_f16, int T, int K, int N, int group, int bmax, const uint32_t counts[9],
+                                    const uint32_t* segs, const void* scales_f16, const void* zeros_f16, float* y,
+                                    void* workspace, size_t workspace_bytes, void* stream) {
+    if (!y || !x_f16 || !counts) return GRINQH_ERR_NULL;
+    if (((uintptr_t)y | (uintptr_t)x_f16) & 15) return GRINQH_ERR_ALIGN;
+    if (T != 1 || N % 128 || (bmax != 4 && bmax != 6 && bmax != 8)) return GRINQH_ERR_SHAPE;
+    const int rc = gq::check_vmm_ptrs(T, K, N, group, segs, scales_f16, zeros_f16, x_f16, x_f16, workspace,
+                                      workspace_bytes);
+    if (rc != GRINQH_OK) return rc;
+    unsigned long long total = 0;
+    for (int w = 0; w < 9; ++w) {
+        total += counts[w];
+        if (counts[w] && ((w & 1) || w > bmax)) return GRINQH_ERR_MIX;  // widths are 0, 2, .., b_max
+    }
+    if (total != (unsigned long long)K) return GRINQH_ERR_MIX;
+    gq::VmmArgs a{T, K, N, 1, gq::MODE_RANK, bmax, segs, scales_f16, zeros_f16, nullptr, nullptr, (const uint16_t*)x_f16,
+                  gq::cuts_from_counts(counts), workspace, y, (cudaStream_t)stream};
+    const gq::VmmPlan pl = gq::vmm_plan(T, K, N);
+    return gq::launch_impl<1, 16, true, gq::MODE_RANK, false, true>(a, pl);
 }

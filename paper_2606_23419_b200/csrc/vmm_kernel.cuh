@@ -82,6 +82,7 @@ struct VmmPlan {
 
 struct VmmArgs {
     int T, K, N, fused, mode;
+    int bmax;  // 8 for the 1-bit plane store; 4 / 6 / 8 for the 2-bit-segment store
     const uint32_t* planes;
     const void *scales, *zeros;
     const uint32_t* gsched;
@@ -147,9 +148,9 @@ __device__ __forceinline__ void accumulate_row(const uint32_t (&V)[8], uint16_t 
 // gsched[t][g*128 + p] (MODE_SCHED, written by grinqh_assign) is position p of group g's list for token t:
 //   bits 0..7 local row r | 8..11 b_t (token's width) | 12..15 b (union width = planes fetched) | 16..31 x_t[r] fp16
 // The in-kernel forms build the same entries from xraw.
-template <int T, int VW, bool A16, int MODE, bool BULK>
+template <int T, int VW, bool A16, int MODE, bool BULK, bool SEG2>
 __global__ void __launch_bounds__(VW * 32, 1)
-vmm_kernel(int K, int N, int Sx, int fused, const uint32_t* __restrict__ planes, const __half* __restrict__ scales,
+vmm_kernel(int K, int N, int Sx, int fused, int bmax, const uint32_t* __restrict__ planes, const __half* __restrict__ scales,
            const __half* __restrict__ zeros, const uint32_t* __restrict__ gsched, const uint8_t* __restrict__ gcnt_ge,
            const uint16_t* __restrict__ xraw, CutParams cp, float* __restrict__ part, int* __restrict__ tickets,
            float* __restrict__ y) {
@@ -166,8 +167,10 @@ vmm_kernel(int K, int N, int Sx, int fused, const uint32_t* __restrict__ planes,
     const int words = N >> 5;
     const int word = tile * 32 + lane;
     const bool active = word < words;
-    const uint32_t rowbytes = (uint32_t)words * 4u;
-    const size_t pbytes = (size_t)K * rowbytes;  // one plane
+    // bytes of one row of one plane (or of one 2-bit segment: twice as many), and of one whole plane / segment
+    const uint32_t rowbytes = (uint32_t)words * (SEG2 ? 8u : 4u);
+    const size_t pbytes = (size_t)K * rowbytes;
+    static_assert(!SEG2 || (T == 1 && A16 && !BULK), "the 2-bit-segment store: one token, aligned rows, cp.async copies");
     const int groups = K / GQ_G;
     const int nd = cp.nd;
 
@@ -178,6 +181,8 @@ vmm_kernel(int K, int N, int Sx, int fused, const uint32_t* __restrict__ planes,
     uint16_t* s_tie = reinterpret_cast<uint16_t*>(smem + C::BASE_BYTES);  // [T][groups][8] ordered tie offsets
 
 #ifdef GQ_TIMING
+    unsigned long long gt0, gt2 = 0;
+    asm volatile("mov.u64 %0, %globaltimer;" : "=l"(gt0));
     long long stamp[16];
     int nst = 0;
 #define GQ_STAMP() stamp[nst++] = clock64()
@@ -308,14 +313,19 @@ vmm_kernel(int K, int N, int Sx, int fused, const uint32_t* __restrict__ planes,
     __syncthreads();  // from here on the warp regions belong to their warps
     GQ_STAMP();
 
-    // per-lane copy geometry: lane copies chunk `seg` (16 B) of plane pj (and pj + 4); pjx = 99 disables the lane
-    const int pj = lane >> 3, seg = lane & 7;
-    const bool chunk_ok = A16 ? (tile * 32 + seg * 4 < words) : active;
+    // per-lane copy geometry: lane copies chunk `seg` (16 B) of plane pj (and pj + 4); pjx = 99 disables the lane.
+    // 2-bit segments: a segment row of the tile is 256 B: lanes 16 j .. 16 j + 15 copy segment j (and j + 2).
+    const int pj = SEG2 ? (lane >> 4) : (lane >> 3), seg = SEG2 ? (lane & 15) : (lane & 7);
+    const bool chunk_ok = SEG2 ? (tile * 64 + seg * 4 < 2 * words) : A16 ? (tile * 32 + seg * 4 < words) : active;
     const int pjx = chunk_ok ? (A16 ? pj : 0) : 99;
     const uint8_t* lane_src = reinterpret_cast<const uint8_t*>(planes) +
-                              (A16 ? (size_t)pj * pbytes + (size_t)(tile * 32 + seg * 4) * 4 : (size_t)word * 4);
-    const uint32_t lane_dst = A16 ? ring_s + pj * 128 + seg * 16 : ring_s + lane * 4;
-    const size_t hi_off = 4 * pbytes;  // planes 4..7 of the same row
+                              (SEG2 ? (size_t)pj * pbytes + (size_t)(tile * 64 + seg * 4) * 4
+                               : A16 ? (size_t)pj * pbytes + (size_t)(tile * 32 + seg * 4) * 4
+                                     : (size_t)word * 4);
+    const uint32_t lane_dst = SEG2 ? ring_s + pj * 256 + seg * 16 : A16 ? ring_s + pj * 128 + seg * 16 : ring_s + lane * 4;
+    const size_t hi_off = (SEG2 ? 2 : 4) * pbytes;  // planes 4..7 (segments 2, 3) of the same row
+    // 2-bit segments with b_max < 8: the codes are left-aligned in the byte, so everything is 2^(8 - b_max) too large
+    const float code_scale = SEG2 ? CODE_SCALE / (float)(1 << (8 - bmax)) : CODE_SCALE;
     // bulk-copy form: lane j copies the whole 128-byte segment of plane j with one cp.async.bulk; slot v mod RING has
     // its own mbarrier (one arrival = the expect_tx of lane 0, then the bytes)
     const uint32_t mbar_s = (uint32_t)__cvta_generic_to_shared(wbase + C::MBAR_OFF);
@@ -454,7 +464,10 @@ vmm_kernel(int K, int N, int Sx, int fused, const uint32_t* __restrict__ planes,
                 if (b > 0) {
                     const float xf = __half2float(__ushort_as_half((uint16_t)(ww >> 16)));
                     Xp[t] += xf;
-                    Pp[t] = fmaf(xf, (float)(0x80 >> b), Pp[t]);  // phi_b = 2^(7-b), phi_8 = 0
+                    // phi_b = 2^(7-b), phi_8 = 0; 2-bit segments: in the left-aligned byte, 0 at b = b_max
+                    const float ph = SEG2 ? ((b == bmax) ? 0.f : (float)(0x80 >> b) / (float)(1 << (8 - bmax)))
+                                          : (float)(0x80 >> b);
+                    Pp[t] = fmaf(xf, ph, Pp[t]);
                 }
             }
         }
@@ -528,7 +541,10 @@ vmm_kernel(int K, int N, int Sx, int fused, const uint32_t* __restrict__ planes,
                 const int b = (e.x >> 12) & 15;
                 const uint8_t* src = lane_src + e.y;
                 const uint32_t dst = lane_dst + so;
-                if (A16) {
+                if (SEG2) {
+                    if (2 * pjx < b) cp_async16(dst, src);
+                    if (2 * pjx + 4 < b) cp_async16(dst + 512, src + hi_off);
+                } else if (A16) {
                     if (pjx < b) cp_async16(dst, src);
                     if (pjx + 4 < b) cp_async16(dst + 512, src + hi_off);
                 } else {
@@ -645,6 +661,31 @@ vmm_kernel(int K, int N, int Sx, int fused, const uint32_t* __restrict__ planes,
         }
     };
 
+    // one row of the 2-bit-segment store: NS segments of 2 x 16 columns -> 32 left-aligned codes -> 32 FMAs
+    auto consume2 = [&](auto ns_tag, uint32_t m, int v) {
+        constexpr int NS = decltype(ns_tag)::value;
+        const uint2* slot = reinterpret_cast<const uint2*>(ring + (uint32_t)(v & (RING - 1)) * SLOT_BYTES) + lane;
+        uint32_t a0[4] = {0u, 0u, 0u, 0u}, a1[4] = {0u, 0u, 0u, 0u}, X0[4], X1[4];
+#pragma unroll
+        for (int sg = 0; sg < NS; ++sg) {
+            const uint2 w = slot[sg * 32];
+            a0[sg] = w.x;
+            a1[sg] = w.y;
+        }
+        gather_seg2<NS>(a0, X0);
+        gather_seg2<NS>(a1, X1);
+        const uint16_t xh = (uint16_t)(m >> 16);
+#pragma unroll
+        for (int r = 0; r < 8; ++r) {  // column r of the half = byte r >> 2 of X[r & 3], column 8 + r = byte (r >> 2) + 2
+            const uint32_t h01 = (r < 4) ? __byte_perm(X0[r & 3], 0u, 0x4240) : __byte_perm(X0[r & 3], 0u, 0x4341);
+            const uint32_t h23 = (r < 4) ? __byte_perm(X1[r & 3], 0u, 0x4240) : __byte_perm(X1[r & 3], 0u, 0x4341);
+            fhfma_lo(acc[0][4 * r + 0], h01, xh);
+            fhfma_hi(acc[0][4 * r + 1], h01, xh);
+            fhfma_lo(acc[0][4 * r + 2], h23, xh);
+            fhfma_hi(acc[0][4 * r + 3], h23, xh);
+        }
+    };
+
     // scale/zero chunk L of the segment: columns 8L..8L+7 of the lane (acc[4r + L], r = 0..7) leave the accumulators
     auto chunk = [&](auto l_tag, uint32_t e, int v) {
         constexpr int L = decltype(l_tag)::value;
@@ -674,7 +715,7 @@ vmm_kernel(int K, int N, int Sx, int fused, const uint32_t* __restrict__ planes,
 #pragma unroll
                 for (int r = 0; r < 8; ++r) {
                     float* dst = yacc + t * YSLOT + (8 * L + r) * 33 + lane;
-                    *dst = fmaf(zf[r], X[t], fmaf(sf[r], fmaf(acc[t][4 * r + L], CODE_SCALE, Phi[t]), *dst));
+                    *dst = fmaf(zf[r], X[t], fmaf(sf[r], fmaf(acc[t][4 * r + L], code_scale, Phi[t]), *dst));
                 }
         }
 #pragma unroll
@@ -702,7 +743,8 @@ vmm_kernel(int K, int N, int Sx, int fused, const uint32_t* __restrict__ planes,
                 do {
                     wait_entry(cv);
                     issue_one();
-                    consume(b_tag, e, cv);
+                    if constexpr (SEG2) consume2(integral_constant<int, (B >= 2 ? B / 2 : 1)>{}, e, cv);
+                    else consume(b_tag, e, cv);
                     ++cv;
                     e = list[cv & (LN - 1)].x;
                 } while (cv < stop && !(e & ENTRY_SZ) &&
@@ -724,6 +766,7 @@ vmm_kernel(int K, int N, int Sx, int fused, const uint32_t* __restrict__ planes,
                 if (b == 8) run(integral_constant<int, 8>{});
                 else if (b == 4) run(integral_constant<int, 4>{});
                 else if (b == 2) run(integral_constant<int, 2>{});
+                else if constexpr (SEG2) run(integral_constant<int, 6>{});  // (widths are 2, 4, 6, 8 there)
                 else run(integral_constant<int, 0>{});
             }
         }
@@ -789,8 +832,10 @@ vmm_kernel(int K, int N, int Sx, int fused, const uint32_t* __restrict__ planes,
         }
     }
 #ifdef GQ_TIMING
+    asm volatile("mov.u64 %0, %globaltimer;" : "=l"(gt2));
+    if (tid == 0) printf("CTA %d %d %llu %llu\n", blockIdx.x, blockIdx.y, gt0, gt2);
     GQ_STAMP();
-    if (lane == 0 && (warp == 0 || warp == VW - 1) && blockIdx.x == 0 && (blockIdx.y == 0 || blockIdx.y == gridDim.y - 1)) {
+    if (false && lane == 0 && (warp == 0 || warp == VW - 1) && blockIdx.x == 0 && (blockIdx.y == 0 || blockIdx.y == gridDim.y - 1)) {
         if (MODE == MODE_RANK && warp == 0 && blockIdx.y == 0) {
             printf("select:");
             for (int i = 1; i < g_sel_n; ++i) printf(" %lld", g_sel_stamp[i] - g_sel_stamp[0]);
@@ -808,17 +853,18 @@ vmm_kernel(int K, int N, int Sx, int fused, const uint32_t* __restrict__ planes,
 __global__ void __launch_bounds__(256)
 vmm_reduce_kernel(const float* __restrict__ part, int S, int T, int N, float* __restrict__ y);
 
-template <int T, int VW, bool A16, int MODE, bool BULK = false>
+template <int T, int VW, bool A16, int MODE, bool BULK = false, bool SEG2 = false>
 static int launch_impl(const VmmArgs& a, const VmmPlan& pl) {
     using C = Cfg<T, VW>;
     const size_t smem = (size_t)C::BASE_BYTES + (MODE == MODE_SCHED ? 0 : (size_t)T * (a.K / GQ_G) * 16);
     // the attribute belongs to the device: set it on every launch (cheap, legal during stream capture)
-    if (cudaFuncSetAttribute(vmm_kernel<T, VW, A16, MODE, BULK>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) !=
+    if (cudaFuncSetAttribute(vmm_kernel<T, VW, A16, MODE, BULK, SEG2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) !=
         cudaSuccess)
         return GRINQH_ERR_CUDA;
     dim3 grid(pl.col_tiles, pl.Sx);
     const cudaError_t e =
-        launch_pdl(vmm_kernel<T, VW, A16, MODE, BULK>, grid, dim3(C::NT), smem, a.st, a.K, a.N, pl.Sx, a.fused, a.planes,
+        launch_pdl(vmm_kernel<T, VW, A16, MODE, BULK, SEG2>, grid, dim3(C::NT), smem, a.st, a.K, a.N, pl.Sx, a.fused, a.bmax,
+                   a.planes,
                    (const __half*)a.scales, (const __half*)a.zeros, a.gsched, a.gcnt_ge, a.xraw, a.cp,
                    (float*)((char*)a.workspace + TICKET_BYTES), (int*)a.workspace, a.y);
     return e == cudaSuccess ? GRINQH_OK : GRINQH_ERR_CUDA;

@@ -24,8 +24,29 @@ int check(unsigned seed) {
     return 0;
 }
 
+// 2-bit-segment store: X[j] byte i = left-aligned code of column 4 i + j, from NS segment words of 16 pairs each
+template <int NS>
+int check2(unsigned seed) {
+    srand(seed);
+    for (int it = 0; it < 2000; ++it) {
+        uint32_t a[4], X[4];
+        for (int j = 0; j < 4; ++j) a[j] = ((uint32_t)rand() << 17) ^ ((uint32_t)rand() << 5) ^ (uint32_t)rand();
+        gq::gather_seg2<NS>(a, X);
+        for (int c = 0; c < 16; ++c) {
+            int code = 0;
+            for (int sg = 0; sg < NS; ++sg) code |= (int)((a[sg] >> (2 * c)) & 3u) << (6 - 2 * sg);
+            int got = (int)((X[c & 3] >> (8 * (c >> 2))) & 0xFFu);
+            if (got != code) {
+                printf("FAIL seg2 NS=%d c=%d code=%d got=%d\n", NS, c, code, got);
+                return 1;
+            }
+        }
+    }
+    return 0;
+}
+
 int main() {
-    int rc = check<2>(1) | check<4>(2) | check<8>(3);
+    int rc = check<2>(1) | check<4>(2) | check<8>(3) | check2<1>(4) | check2<2>(5) | check2<3>(6) | check2<4>(7);
     if (!rc) printf("OK\n");
     return rc;
 }

@@ -569,3 +569,67 @@ def test_repeatability_under_reuse(gq):
                 _check_y(y, y_ref)
                 first[i] = y
             assert np.array_equal(y, first[i]), (rnd, i)
+
+
+# ---- the paper's 2-bit-segment store, b_max in {4, 6, 8}
+SEG2_MIXES = {4: [0.125, 0, 0.375, 0, 0.5, 0, 0, 0, 0], 6: [0.125, 0, 0.25, 0, 0.375, 0, 0.25, 0, 0],
+              8: [0.125, 0, 0.25, 0, 0.25, 0, 0.125, 0, 0.25]}
+
+
+@pytest.mark.parametrize("bmax", [4, 6, 8])
+@pytest.mark.parametrize("K,N,seed", [(256, 512, 0), (384, 1184, 1), (128, 32, 2)])
+def test_pack_seg2_bit_exact(gq, bmax, K, N, seed):
+    W = synth.make_weights(K, N, 0.02, seed)
+    W[:128, 0] = np.float16(0.25)                       # constant group
+    W[:128, 1] = np.float16(-0.0)
+    segs, s, z = oracle.pack2(W, bmax)
+    out = gq.grinqh_pack_seg2(_dev(W), bmax)
+    torch.cuda.synchronize()
+    assert np.array_equal(out.segs.cpu().numpy().view(np.uint32), segs)
+    assert np.array_equal(out.scales.cpu().numpy().view(np.uint16), s.view(np.uint16))
+    assert np.array_equal(out.zeros.cpu().numpy().view(np.uint16), z.view(np.uint16))
+
+
+@pytest.mark.parametrize("bmax", [4, 6, 8])
+@pytest.mark.parametrize("K,N,dist,seed", [(256, 512, "normal", 0), (1024, 2176, "student_t", 1), (2048, 4096, "normal", 2),
+                                           (512, 128, "student_t", 3)])
+def test_vmm_rank_seg2_matches_oracle(gq, bmax, K, N, dist, seed):
+    """rank assignment (widths 0, 2, .., b_max) + selective SEGMENT fetch + reconstruction with the store's own b_max"""
+    W = synth.make_weights(K, N, 0.02, 40 + seed)
+    x = synth.make_x(1, K, 50 + seed, dist)
+    counts = oracle.mix_to_counts(K, SEG2_MIXES[bmax])
+    segs, s, z = oracle.pack2(W, bmax)
+    bits = oracle.assign(x, counts)["bits"]
+    y_ref = oracle.vmm2(x, segs, s, z, bits, bmax)
+    w = gq.grinqh_pack_seg2(_dev(W), bmax)
+    y = gq.grinqh_vmm_rank_seg2(_dev(x), counts, w).cpu().numpy()
+    _check_y(y, y_ref, bmax)
+    if bmax == 8:       # the same weights in the 1-bit plane store give the same y up to the summation order
+        y_planes = gq.grinqh_vmm_rank(_dev(x), counts, gq.grinqh_pack(_dev(W))).cpu().numpy()
+        _check_y(y, y_planes.astype(np.float64), "planes")
+    with pytest.raises(gq.GrinqhError):
+        gq.grinqh_vmm_rank_seg2(_dev(x), oracle.mix_to_counts(K, synth.MIXES["4"] if bmax < 8 else
+                                                             [0.5, 0.5, 0, 0, 0, 0, 0, 0, 0]), w)
+
+
+def test_vmm_rank_seg2_full_size_sampled_columns(gq):
+    """4096 x 28672 (gate|up) over the b_max = 8 segment store, avg-4 mix, oracle on sampled columns"""
+    K, N, bmax = 4096, 28672, 8
+    g = torch.Generator(device="cuda")
+    g.manual_seed(99)
+    Wd = (torch.randn((K, N), generator=g, device="cuda", dtype=torch.float32) * 0.02).to(torch.float16)
+    x = synth.make_x(1, K, 78, "normal")
+    counts = oracle.mix_to_counts(K, synth.MIXES["4"])
+    w = gq.grinqh_pack_seg2(Wd, bmax)
+    y = gq.grinqh_vmm_rank_seg2(_dev(x), counts, w).cpu().numpy()
+    cols = np.unique(np.concatenate([np.arange(0, 32), np.arange(N - 32, N),
+                                     np.random.default_rng(1).integers(0, N, 96)])).astype(np.int32)
+    blocks = np.unique(cols // 16)
+    Wh = Wd[:, torch.from_numpy(np.concatenate([np.arange(b * 16, (b + 1) * 16) for b in blocks])).cuda()].cpu().numpy()
+    segs, s, z = oracle.pack2(np.ascontiguousarray(Wh), bmax)
+    gs = w.segs[:, :, torch.from_numpy(blocks.astype(np.int64)).cuda()].cpu().numpy().view(np.uint32)
+    assert np.array_equal(gs, segs)
+    remap = {int(b): i for i, b in enumerate(blocks)}
+    sub_cols = np.array([remap[int(c) // 16] * 16 + int(c) % 16 for c in cols], np.int32)
+    y_ref = oracle.vmm2(x, segs, s, z, oracle.assign(x, counts)["bits"], bmax, cols=sub_cols)
+    _check_y(y[:, cols], y_ref)
