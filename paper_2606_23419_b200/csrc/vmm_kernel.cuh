@@ -793,18 +793,24 @@ vmm_kernel(int K, int N, int Sx, int fused, int bmax, const uint32_t* __restrict
             }
         }
     if (fused && Sx > 1) {
+        GQ_STAMP();
         __syncthreads();  // the CTA's partial is complete ...
+        GQ_STAMP();
         if (tid == 0) {
-            __threadfence();  // ... and (fence cumulativity over the barrier) visible device-wide before its ticket
-            const int last = (atomicAdd(&tickets[tile], 1) == Sx - 1);
-            if (last) __threadfence();  // acquire side: the other CTAs' partials, read below with ld.global.cg
-            s_last = last;
+            // ... and released device-wide with the ticket: ONE acq_rel atomic (release: the CTA's partial, ordered
+            // before it by the barrier; acquire: the other CTAs' partials for the last one) instead of a sequentially
+            // consistent fence on either side of a relaxed atomic
+            int old;
+            asm volatile("atom.add.acq_rel.gpu.global.s32 %0, [%1], 1;" : "=r"(old) : "l"(tickets + tile) : "memory");
+            s_last = (old == Sx - 1);
         }
+        GQ_STAMP();
         __syncthreads();
+        GQ_STAMP();
         if (s_last) {
-            // float2 columns spread over all the CTA's threads, 16 partials per column in flight, added in the fixed
+            // float2 columns spread over all the CTA's threads, 32 partials per column in flight, added in the fixed
             // order s = 0..Sx-1
-            constexpr int BATCH = 16;
+            constexpr int BATCH = 32;
 #pragma unroll 1
             for (int t = 0; t < T; ++t)
 #pragma unroll 1
@@ -833,15 +839,14 @@ vmm_kernel(int K, int N, int Sx, int fused, int bmax, const uint32_t* __restrict
     }
 #ifdef GQ_TIMING
     asm volatile("mov.u64 %0, %globaltimer;" : "=l"(gt2));
-    if (tid == 0) printf("CTA %d %d %llu %llu\n", blockIdx.x, blockIdx.y, gt0, gt2);
     GQ_STAMP();
-    if (false && lane == 0 && (warp == 0 || warp == VW - 1) && blockIdx.x == 0 && (blockIdx.y == 0 || blockIdx.y == gridDim.y - 1)) {
-        if (MODE == MODE_RANK && warp == 0 && blockIdx.y == 0) {
+    if (tid == 0 && (s_last == 1 || blockIdx.y == 0) && blockIdx.x == 0) {
+        if (false) {
             printf("select:");
             for (int i = 1; i < g_sel_n; ++i) printf(" %lld", g_sel_stamp[i] - g_sel_stamp[0]);
             printf("\n");
         }
-        printf("blk %3d warp %2d entries %3d:", blockIdx.y, warp, cv);
+        printf("blk %3d last %d entries %3d:", blockIdx.y, s_last, cv);
         for (int i = 1; i < nst; ++i) printf(" %6lld", stamp[i] - stamp[0]);
         printf("\n");
     }
