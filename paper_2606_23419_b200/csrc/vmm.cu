@@ -1,5 +1,7 @@
-// vmm.cu — C ABI of the VMM (grinqh_vmm, grinqh_vmm_rank, grinqh_vmm_thresholds, the two-launch form), the
-// shape-only launch plan and the one-token instantiations of the kernel in vmm_kernel.cuh.
+// vmm.cu — C ABI of the VMM (grinqh_vmm, grinqh_vmm_rank, grinqh_vmm_thresholds, the two-launch form, the 2-bit-segment
+// form), the routing between the two kernel families (vmm_args.cuh), the stream kernel's shape-only plan and its
+// one-token instantiations (vmm_kernel.cuh).
+#include <algorithm>
 #include <cstdlib>
 
 #include "vmm_kernel.cuh"
@@ -19,7 +21,7 @@ vmm_reduce_kernel(const float* __restrict__ part, int S, int T, int N, float* __
     *reinterpret_cast<float4*>(y + (size_t)t * N + n) = a;
 }
 
-static int num_sms() {
+int num_sms() {
     static int cached[64];
     int dev = 0;
     if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return 148;
@@ -105,7 +107,9 @@ static int launch_t1(const VmmArgs& a, const VmmPlan& pl) {
     }
 }
 
-static int launch_vmm(const VmmArgs& a) {
+int stream_sx(int T, int K, int N) { return vmm_plan(T, K, N).Sx; }
+
+int launch_vmm_stream(const VmmArgs& a) {
     const VmmPlan pl = vmm_plan(a.T, a.K, a.N);
     if (a.T > 1) return launch_vmm_multi(a, pl);
     switch (a.mode) {
@@ -114,6 +118,23 @@ static int launch_vmm(const VmmArgs& a) {
         default: return launch_t1<MODE_RANK>(a, pl);
     }
 }
+
+// The 1-bit plane store goes to the item kernel (vmm_items.cu): at every shape of the configs it is the faster of the
+// two (profiles/r02_kernels.md).  GRINQH_STREAM=1 (read once) routes it to the stream kernel instead — the A/B switch
+// of that table, and what GRINQH_BULK=1 needs.
+static bool use_stream() {
+    static int v = -1;
+    if (v < 0) {
+        const char* f = getenv("GRINQH_STREAM");
+        v = ((f && atoi(f) == 1) || use_bulk()) ? 1 : 0;
+    }
+    return v != 0;
+}
+
+static int launch_vmm(const VmmArgs& a) { return use_stream() ? launch_vmm_stream(a) : launch_vmm_items(a); }
+
+// split-K partials per column tile of the launch that `mode` gets (the two-launch form reads it back)
+static int active_sx(int T, int K, int N, int mode) { return use_stream() ? stream_sx(T, K, N) : items_sx(T, K, N, mode); }
 
 static int check_vmm_args(int T, int K, int N, int group) {
     if (group != GQ_G || T < 1 || T > GRINQH_MAX_T || K <= 0 || N <= 0 || K % GQ_G || N % 32 || K > GQ_MAX_K)
@@ -138,8 +159,11 @@ static int check_vmm_ptrs(int T, int K, int N, int group, const void* planes, co
 
 extern "C" size_t grinqh_vmm_workspace_bytes(int T, int K, int N) {
     if (gq::check_vmm_args(T, K, N, GQ_G) != GRINQH_OK) return 0;
-    const gq::VmmPlan pl = gq::vmm_plan(T, K, N);
-    return gq::TICKET_BYTES + (size_t)pl.Sx * T * N * sizeof(float);
+    // one workspace serves every entry point: the largest split-K factor of the plans behind them
+    int sx = gq::stream_sx(T, K, N);
+    sx = std::max(sx, gq::items_sx(T, K, N, gq::MODE_SCHED));
+    sx = std::max(sx, gq::items_sx(T, K, N, gq::MODE_RANK));
+    return gq::TICKET_BYTES + (size_t)sx * T * N * sizeof(float);
 }
 
 extern "C" int grinqh_vmm_workspace_init(void* workspace, size_t workspace_bytes, void* stream) {
@@ -181,10 +205,9 @@ extern "C" int grinqh_vmm_reduce(int T, int K, int N, float* y, const void* work
     if (rc != GRINQH_OK) return rc;
     if (((uintptr_t)y | (uintptr_t)workspace) & 15) return GRINQH_ERR_ALIGN;
     if (workspace_bytes < grinqh_vmm_workspace_bytes(T, K, N)) return GRINQH_ERR_WORKSPACE;
-    const gq::VmmPlan pl = gq::vmm_plan(T, K, N);
     dim3 grid((N + 4 * 256 - 1) / (4 * 256), T);
     gq::vmm_reduce_kernel<<<grid, 256, 0, (cudaStream_t)stream>>>(
-        (const float*)((const char*)workspace + gq::TICKET_BYTES), pl.Sx, T, N, y);
+        (const float*)((const char*)workspace + gq::TICKET_BYTES), gq::active_sx(T, K, N, gq::MODE_SCHED), T, N, y);
     return cudaGetLastError() == cudaSuccess ? GRINQH_OK : GRINQH_ERR_CUDA;
 }
 

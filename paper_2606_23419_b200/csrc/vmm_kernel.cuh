@@ -39,6 +39,7 @@
 #include "common.cuh"
 #include "gather.cuh"
 #include "select.cuh"
+#include "vmm_args.cuh"
 
 namespace gq {
 
@@ -48,9 +49,7 @@ constexpr int YSLOT = 32 * 33;     // one warp's 1024 sums, padded: column 32*l 
 constexpr int GLC = 8;             // group lists a CTA builds once for all its warps (one token, in-kernel assignment)
 constexpr int MAXG = GQ_MAX_K / GQ_G;
 constexpr uint32_t ENTRY_SZ = 0x80u;  // list entry is a scale/zero chunk (bits 0..1 = chunk); rows use bits 0..6
-constexpr size_t TICKET_BYTES = 16384;  // head of the workspace: one int per column tile, zero between launches
 
-enum { MODE_SCHED = 0, MODE_THR = 1, MODE_RANK = 2 };
 
 constexpr int cmax(int a, int b) { return a > b ? a : b; }
 
@@ -80,19 +79,6 @@ struct VmmPlan {
     int vw;         // warps per CTA
 };
 
-struct VmmArgs {
-    int T, K, N, fused, mode;
-    int bmax;  // 8 for the 1-bit plane store; 4 / 6 / 8 for the 2-bit-segment store
-    const uint32_t* planes;
-    const void *scales, *zeros;
-    const uint32_t* gsched;
-    const uint8_t* gcnt_ge;
-    const uint16_t* xraw;
-    CutParams cp;
-    void* workspace;
-    float* y;
-    cudaStream_t st;
-};
 
 // codes are fed to the FMA as fp16 bit patterns 0x00cc = cc * 2^-24 (subnormal halfs, exact)
 constexpr float CODE_SCALE = 16777216.0f;
