@@ -23,9 +23,19 @@ def _deps():
     return glob.glob(os.path.join(CSRC, "*.cuh")) + [os.path.join(HERE, "..", "include", "grinqh.h")]
 
 
+def _tag() -> str:
+    return "_".join(e.strip("-") for e in os.environ.get("GQ_NVCC_EXTRA", "").split())
+
+
 def needs_build() -> bool:
     if not os.path.exists(LIB):
         return True
+    try:  # the library on disk was linked from objects built with other extra flags
+        if open(LIB + ".tag").read() != _tag():
+            return True
+    except OSError:
+        if _tag():
+            return True
     t = os.path.getmtime(LIB)
     return any(os.path.getmtime(d) > t for d in sources() + _deps())
 
@@ -35,7 +45,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
         return LIB
     os.makedirs(OBJ, exist_ok=True)
     extra = os.environ.get("GQ_NVCC_EXTRA", "").split()
-    tag = "_".join(e.strip("-") for e in extra)
+    tag = _tag()
     hdr_t = max(os.path.getmtime(d) for d in _deps())
 
     def compile_one(src):
@@ -49,6 +59,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     with ThreadPoolExecutor(max_workers=8) as ex:
         objs = list(ex.map(compile_one, sources()))
     subprocess.check_call([NVCC, "--shared", "-cudart", "static", "-o", LIB] + objs)
+    with open(LIB + ".tag", "w") as f:
+        f.write(tag)
     return LIB
 
 

@@ -133,8 +133,8 @@ static bool use_stream() {
 
 static int launch_vmm(const VmmArgs& a) { return use_stream() ? launch_vmm_stream(a) : launch_vmm_items(a); }
 
-// split-K partials per column tile of the launch that `mode` gets (the two-launch form reads it back)
-static int active_sx(int T, int K, int N, int mode) { return use_stream() ? stream_sx(T, K, N) : items_sx(T, K, N, mode); }
+// split-K partials per column tile of the launch (the two-launch form reads it back)
+static int active_sx(int T, int K, int N) { return use_stream() ? stream_sx(T, K, N) : items_sx(T, K, N); }
 
 static int check_vmm_args(int T, int K, int N, int group) {
     if (group != GQ_G || T < 1 || T > GRINQH_MAX_T || K <= 0 || N <= 0 || K % GQ_G || N % 32 || K > GQ_MAX_K)
@@ -161,8 +161,7 @@ extern "C" size_t grinqh_vmm_workspace_bytes(int T, int K, int N) {
     if (gq::check_vmm_args(T, K, N, GQ_G) != GRINQH_OK) return 0;
     // one workspace serves every entry point: the largest split-K factor of the plans behind them
     int sx = gq::stream_sx(T, K, N);
-    sx = std::max(sx, gq::items_sx(T, K, N, gq::MODE_SCHED));
-    sx = std::max(sx, gq::items_sx(T, K, N, gq::MODE_RANK));
+    sx = std::max(sx, gq::items_sx(T, K, N));
     return gq::TICKET_BYTES + (size_t)sx * T * N * sizeof(float);
 }
 
@@ -207,7 +206,7 @@ extern "C" int grinqh_vmm_reduce(int T, int K, int N, float* y, const void* work
     if (workspace_bytes < grinqh_vmm_workspace_bytes(T, K, N)) return GRINQH_ERR_WORKSPACE;
     dim3 grid((N + 4 * 256 - 1) / (4 * 256), T);
     gq::vmm_reduce_kernel<<<grid, 256, 0, (cudaStream_t)stream>>>(
-        (const float*)((const char*)workspace + gq::TICKET_BYTES), gq::active_sx(T, K, N, gq::MODE_SCHED), T, N, y);
+        (const float*)((const char*)workspace + gq::TICKET_BYTES), gq::active_sx(T, K, N), T, N, y);
     return cudaGetLastError() == cudaSuccess ? GRINQH_OK : GRINQH_ERR_CUDA;
 }
 

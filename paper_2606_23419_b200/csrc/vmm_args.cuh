@@ -28,7 +28,7 @@ struct VmmArgs {
 };
 
 int num_sms();                              // of the current device
-int items_sx(int T, int K, int N, int mode);  // split-K partials per column tile of the item kernel's plan (MODE_*)
+int items_sx(int T, int K, int N);          // split-K partials per column tile of the item kernel's plan
 int launch_vmm_items(const VmmArgs& a);     // vmm_items.cu
 int stream_sx(int T, int K, int N);         // ... of the stream kernel's plan
 int launch_vmm_stream(const VmmArgs& a);    // vmm.cu / vmm_multi.cu

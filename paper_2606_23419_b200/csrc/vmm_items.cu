@@ -46,7 +46,6 @@ constexpr int VTHREADS = VW * 32;
 constexpr int TILE_COLS = 1024;
 constexpr int SLOT_BYTES = 1024;   // 8 planes x 128 B
 constexpr int YSLOT = 32 * 33;     // one warp's 1024 sums, padded: column 32*l + c lives at c*33 + l
-constexpr int ctas_per_sm(int T) { return T <= 2 ? 2 : 1; }  // register / shared-memory budget
 
 template <int T>
 struct Cfg {
@@ -73,9 +72,11 @@ struct VmmPlan {
 // ipw * (rows per item + item overhead), and the launch ends with the last CTA's second pass over Sx partials;
 // pick (warps per CTA, Q in 1..8) that minimises the sum under the residency limit (16 warps per SM either way).
 //
-// rank = the launch selects the cuts itself (grinqh_vmm_rank): the select's histogram and keys (128 KB) alias the warp
-// regions, so one CTA per SM whatever the width, and the 16-warp variant only where its regions plus the tie table fit.
-constexpr int SMEM_LIMIT = 232448;  // 227 KB per CTA
+// ONE plan per shape for every form of the launch (schedule, threshold, rank, two-launch): the forms promise the same
+// bits, and the bits depend on the item partition.  So the plan obeys the rank form's limits — the select's histogram
+// and keys (128 KB) alias the warp regions: one CTA per SM whatever the width, and the 16-warp variant only where its
+// regions plus the tie table fit.
+constexpr int SMEM_LIMIT = 232448 - 1024;  // 227 KB per CTA, static shared memory included (cuts, scratch: < 1 KB)
 static inline int warp_bytes(int T) {
     return T == 1 ? Cfg<1>::WARP_BYTES : T == 2 ? Cfg<2>::WARP_BYTES : T == 3 ? Cfg<3>::WARP_BYTES : Cfg<4>::WARP_BYTES;
 }
@@ -84,14 +85,14 @@ static inline int smem_bytes(int T, int vw, int K, bool rank) {
     return rank ? (base > 2 * 65536 ? base : 2 * 65536) + T * (K / GQ_G) * 16 : base;
 }
 
-static inline VmmPlan vmm_plan(int T, int K, int N, bool rank) {
+static inline VmmPlan vmm_plan(int T, int K, int N) {
     VmmPlan best{};
     const int CT = (N + TILE_COLS - 1) / TILE_COLS;
     const int groups = K / GQ_G;
     double best_cost = 1e30;
     for (int vw = 8; vw <= ((T <= 2) ? 16 : 8); vw *= 2) {
-        if (vw == 16 && smem_bytes(T, vw, K, rank) > SMEM_LIMIT) continue;
-        const int resident = num_sms() * ((vw == 8 && !rank) ? ctas_per_sm(T) : 1);
+        if (vw == 16 && smem_bytes(T, vw, K, true) > SMEM_LIMIT) continue;
+        const int resident = num_sms();
         const int sx_max = resident / CT > 0 ? resident / CT : 1;
         for (int Q = 1; Q <= 16; ++Q) {
             const int I = groups * Q;
@@ -146,7 +147,7 @@ __device__ __forceinline__ void accumulate_row(const uint32_t (&V)[8], uint16_t 
 // fused: the last CTA of a column tile to finish (ticket counter in the workspace, reset to 0 by that CTA) sums the
 // tile's Sx partials in the fixed order s = 0..Sx-1 and writes y: still deterministic, one launch instead of two.
 template <int T, int VWT, bool A16>
-__global__ void __launch_bounds__(VWT * 32, VWT == 8 ? ctas_per_sm(T) : 1)
+__global__ void __launch_bounds__(VWT * 32, 1)
 vmm_items_kernel(int K, int N, int Q, uint32_t rq, int ipw, int Sx, int fused, int mode, const uint32_t* __restrict__ planes,
                 const __half* __restrict__ scales, const __half* __restrict__ zeros,
                 const uint32_t* __restrict__ gsched, const uint8_t* __restrict__ gcnt_ge,
@@ -157,6 +158,8 @@ vmm_items_kernel(int K, int N, int Q, uint32_t rq, int ipw, int Sx, int fused, i
     extern __shared__ __align__(16) uint8_t smem[];
     __shared__ __align__(16) TokenCuts s_tc[T];
     __shared__ SelectScratch s_sel;
+    __shared__ int s_cuts[16];  // Cd[8] | mult[8], read with run-time indices (as kernel parameters every thread would copy
+                                // them to local memory at kernel entry, schedule form included)
     __shared__ int s_last;
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -196,28 +199,35 @@ vmm_items_kernel(int K, int N, int Q, uint32_t rq, int ipw, int Sx, int fused, i
         constexpr int NT = VWT * 32;
         uint32_t* hist = reinterpret_cast<uint32_t*>(smem);
         uint16_t* skeys = reinterpret_cast<uint16_t*>(smem + 65536);
+        if (tid == 0) {
+#pragma unroll
+            for (int d = 0; d < 8; ++d) s_cuts[d] = cp.Cd[d];
+        } else if (tid == 32) {
+#pragma unroll
+            for (int d = 0; d < 8; ++d) s_cuts[8 + d] = cp.mult[d];
+        } else if (tid == 64 && mode != MODE_RANK) {
+#pragma unroll
+            for (int t = 0; t < T; ++t) {
+#pragma unroll
+                for (int d = 0; d < 8; ++d) {
+                    s_tc[t].thr[d] = cp.thr[d];
+                    s_tc[t].take[d] = 0;
+                    s_tc[t].hh[d] = 0;
+                }
+                s_tc[t].split = 0;
+                s_tc[t].nd = nd;
+            }
+        }
         if (mode == MODE_RANK) {  // cleared while the previous kernel is still running
             uint4* z = reinterpret_cast<uint4*>(hist);
             for (int i = tid; i < 4096; i += NT) z[i] = make_uint4(0, 0, 0, 0);
-            __syncthreads();
         }
+        __syncthreads();
         pdl_wait();
 #pragma unroll 1
         for (int t = 0; t < T; ++t) {
-            if (mode == MODE_RANK) {
-                rank_select<NT>(xraw + (size_t)t * K, skeys, K, nd, cp.Cd, hist, t + 1 < T, &s_sel, &s_tc[t]);
-            } else {
-                if (tid < 8) {
-                    s_tc[t].thr[tid] = cp.thr[tid];
-                    s_tc[t].take[tid] = 0;
-                    s_tc[t].hh[tid] = 0;
-                }
-                if (tid == 0) {
-                    s_tc[t].split = 0;
-                    s_tc[t].nd = nd;
-                }
-                __syncthreads();
-            }
+            if (mode == MODE_RANK)
+                rank_select<NT>(xraw + (size_t)t * K, skeys, K, nd, s_cuts, hist, t + 1 < T, &s_sel, &s_tc[t]);
             const uint32_t split = s_tc[t].split;
             if (split) {
                 uint16_t* tie = s_tie + (size_t)t * groups * 8;
@@ -308,7 +318,7 @@ vmm_items_kernel(int K, int N, int Q, uint32_t rq, int ipw, int Sx, int fused, i
             for (int t = 0; t < T; ++t) {
                 int m[4];
                 keys4(xv[t], m);
-                widths4(m, &s_tc[t], cp.mult, nd, s_tie + ((size_t)t * groups + g) * 8, lane, bt[t]);
+                widths4(m, &s_tc[t], s_cuts + 8, nd, s_tie + ((size_t)t * groups + g) * 8, lane, bt[t]);
 #pragma unroll
                 for (int i = 0; i < 4; ++i) bu[i] = max(bu[i], bt[t][i]);
             }
@@ -655,11 +665,11 @@ static int launch_items_impl(const VmmArgs& a, const VmmPlan& pl) {
 
 }  // namespace items
 
-int items_sx(int T, int K, int N, int mode) { return items::vmm_plan(T, K, N, mode == MODE_RANK).Sx; }
+int items_sx(int T, int K, int N) { return items::vmm_plan(T, K, N).Sx; }
 
 int launch_vmm_items(const VmmArgs& a) {
     using namespace items;
-    const VmmPlan pl = vmm_plan(a.T, a.K, a.N, a.mode == MODE_RANK);
+    const VmmPlan pl = vmm_plan(a.T, a.K, a.N);
 #define GQ_LAUNCH_W(TT, WW) \
     return (a.N % 128 == 0) ? launch_items_impl<TT, WW, true>(a, pl) : launch_items_impl<TT, WW, false>(a, pl)
     if (pl.vw == 16) {  // only planned for T <= 2 (registers)
