@@ -51,7 +51,8 @@ typedef enum {
     GRINQH_ERR_ALIGN = -3,     /* a base pointer is not 16-byte aligned                   */
     GRINQH_ERR_MIX = -4,       /* sum(counts) != K                                        */
     GRINQH_ERR_WORKSPACE = -5, /* workspace_bytes smaller than *_workspace_bytes()        */
-    GRINQH_ERR_CUDA = -6       /* a CUDA launch failed; see cudaGetLastError              */
+    GRINQH_ERR_CUDA = -6,      /* a CUDA launch failed; see cudaGetLastError              */
+    GRINQH_ERR_STATIC_LIMIT = -7 /* grinqh_vmm_rank_static: the shape needs more scratch than the static array holds */
 } grinqh_status;
 
 #define GRINQH_GROUP 128
@@ -200,6 +201,26 @@ int grinqh_vmm_thresholds(const void* x_f16, int T, int K, int N, int group, con
 int grinqh_vmm_rank(const void* x_f16, int T, int K, int N, int group, const uint32_t counts[9],
                     const uint32_t* planes, const void* scales_f16, const void* zeros_f16,
                     float* y, void* workspace, size_t workspace_bytes, void* stream);
+
+/*
+ * grinqh_vmm_rank_static — grinqh_vmm_rank (same launch, same bits) for callers that cannot allocate: code under
+ * CUDA graph capture, serving loops and harnesses that forbid cudaMalloc.  The scratch of the launch (ticket counters
+ * + split-K partials, PAPER.md:85 / SURVEY.md 8a4) lives in a file-scope device array of the library instead of a
+ * caller-provided workspace; the call makes no cudaMalloc, cudaFree or allocating library call.
+ *   limit      the array is GRINQH_STATIC_SCRATCH_BYTES of device memory on every GPU that loads the library, held
+ *              until exit; a shape with grinqh_vmm_workspace_bytes(T, K, N) above it returns GRINQH_ERR_STATIC_LIMIT
+ *              (nothing is enqueued) — use grinqh_vmm_rank with a workspace there.
+ *   sharing    every call on a device uses the same array: calls that overlap on the GPU (two streams, graph
+ *              branches without a dependency) RACE; calls ordered on one stream do not.  The tickets are cleared on
+ *              `stream` before every launch; stale partials are never read.
+ *   arguments  as grinqh_vmm_rank without workspace / workspace_bytes; all pointers dev except counts (HOST).
+ * grinqh_static_scratch_bytes returns GRINQH_STATIC_SCRATCH_BYTES as built into the library.
+ */
+#define GRINQH_STATIC_SCRATCH_BYTES (4u << 20)
+size_t grinqh_static_scratch_bytes(void);
+int grinqh_vmm_rank_static(const void* x_f16, int T, int K, int N, int group, const uint32_t counts[9],
+                           const uint32_t* planes, const void* scales_f16, const void* zeros_f16,
+                           float* y, void* stream);
 
 /*
  * The paper's own storage granularity ("decomposed into discrete 2-bit segments",

@@ -54,6 +54,10 @@ _lib.grinqh_vmm_thresholds.restype = _i
 _lib.grinqh_vmm_thresholds.argtypes = [_vp, _i, _i, _i, _i, _vp, _vp, _vp, _vp, _vp, _vp, _sz, _vp]
 _lib.grinqh_vmm_rank.restype = _i
 _lib.grinqh_vmm_rank.argtypes = [_vp, _i, _i, _i, _i, _vp, _vp, _vp, _vp, _vp, _vp, _sz, _vp]
+_lib.grinqh_vmm_rank_static.restype = _i
+_lib.grinqh_vmm_rank_static.argtypes = [_vp, _i, _i, _i, _i, _vp, _vp, _vp, _vp, _vp, _vp]
+_lib.grinqh_static_scratch_bytes.restype = _sz
+_lib.grinqh_static_scratch_bytes.argtypes = []
 _lib.grinqh_pack_seg2.restype = _i
 _lib.grinqh_pack_seg2.argtypes = [_vp, _i, _i, _i, _i, _vp, _vp, _vp, _vp]
 _lib.grinqh_vmm_rank_seg2.restype = _i
@@ -69,7 +73,8 @@ EXPORTS = ("grinqh_status_string", "grinqh_version", "grinqh_mix_to_counts", "gr
            "grinqh_assign_workspace_bytes", "grinqh_assign", "grinqh_assign_thresholds",
            "grinqh_calibrate_thresholds", "grinqh_vmm_workspace_bytes",
            "grinqh_vmm_workspace_init", "grinqh_vmm", "grinqh_vmm_thresholds", "grinqh_vmm_rank",
-           "grinqh_vmm_main", "grinqh_vmm_reduce", "grinqh_decode_host", "grinqh_pack_seg2", "grinqh_vmm_rank_seg2")
+           "grinqh_vmm_main", "grinqh_vmm_reduce", "grinqh_decode_host", "grinqh_pack_seg2", "grinqh_vmm_rank_seg2",
+           "grinqh_static_scratch_bytes", "grinqh_vmm_rank_static")
 
 
 class GrinqhError(RuntimeError):
@@ -248,6 +253,22 @@ def grinqh_vmm_rank(x: torch.Tensor, counts, w: Packed, y: torch.Tensor | None =
     _check(_lib.grinqh_vmm_rank(_dev(x, torch.float16, "x"), T, K, w.N, GROUP, _counts(counts), w.planes.data_ptr(),
                                 w.scales.data_ptr(), w.zeros.data_ptr(), _dev(y, torch.float32, "y"),
                                 workspace.data_ptr(), nbytes, _stream(stream)), "grinqh_vmm_rank")
+    return y
+
+
+def grinqh_static_scratch_bytes() -> int:
+    return int(_lib.grinqh_static_scratch_bytes())
+
+
+def grinqh_vmm_rank_static(x: torch.Tensor, counts, w: Packed, y: torch.Tensor, stream=None) -> torch.Tensor:
+    """grinqh_vmm_rank with the library's static device scratch: allocates nothing, so y is the caller's.
+
+    Shapes whose workspace exceeds grinqh_static_scratch_bytes() raise; calls that overlap on the GPU race on the array.
+    """
+    T, K = x.shape
+    _check(_lib.grinqh_vmm_rank_static(_dev(x, torch.float16, "x"), T, K, w.N, GROUP, _counts(counts),
+                                       w.planes.data_ptr(), w.scales.data_ptr(), w.zeros.data_ptr(),
+                                       _dev(y, torch.float32, "y"), _stream(stream)), "grinqh_vmm_rank_static")
     return y
 
 

@@ -16,6 +16,9 @@ extern "C" const char* grinqh_status_string(int status) {
         case GRINQH_ERR_MIX: return "level mix does not sum to K (or fractions do not sum to 1)";
         case GRINQH_ERR_WORKSPACE: return "workspace too small";
         case GRINQH_ERR_CUDA: return "CUDA launch failed";
+        case GRINQH_ERR_STATIC_LIMIT:
+            return "shape needs more scratch than the library's static array (GRINQH_STATIC_SCRATCH_BYTES); use the "
+                   "workspace form";
         default: return "unknown status";
     }
 }

@@ -42,7 +42,6 @@ namespace gq {
 namespace items {
 
 constexpr int VW = 8;  // warps per CTA (16 in the wide variant: half as many split-K partials, 1 CTA per SM)
-constexpr int VTHREADS = VW * 32;
 constexpr int TILE_COLS = 1024;
 constexpr int SLOT_BYTES = 1024;   // 8 planes x 128 B
 constexpr int YSLOT = 32 * 33;     // one warp's 1024 sums, padded: column 32*l + c lives at c*33 + l
