@@ -241,6 +241,22 @@ int grinqh_vmm_rank_seg2(const void* x_f16, int T, int K, int N, int group, int 
                          float* y, void* workspace, size_t workspace_bytes, void* stream);
 
 /*
+ * grinqh_prefill_gemm — the paper's prefill path ("unpacking the weights at full b_max precision and
+ * performing dense matrix-matrix multiplication", :182 kernel fusion) in one launch:
+ *   Y[M, N] = X[M, K] . W_hat[K, N],  W_hat = s * q + z rounded once to fp16 (exactly what grinqh_unpack writes),
+ * fp16 x fp16 products accumulated in fp32 on the tensor cores (tcgen05, accumulators in TMEM), Y rounded to fp16.
+ * The planes are unpacked inside the kernel into the shared-memory operand tile: HBM sees 1 byte per weight.
+ *   x_f16   dev [M, K] fp16 row-major (any M >= 1; rows beyond M are not read)    y_f16  dev [M, N] fp16 row-major
+ *   planes / scales_f16 / zeros_f16  as written by grinqh_pack
+ * Needs N % 256 == 0, K % 128 == 0, group == 128 (GRINQH_ERR_SHAPE), 16-byte aligned pointers (GRINQH_ERR_ALIGN) and
+ * scales below 128 (weight range per group < 32640: the kernel holds s * 2^9 in fp16).  Enqueued on `stream`; the
+ * tensor map for X is encoded on the host during the call.
+ */
+int grinqh_prefill_gemm(const void* x_f16, int M, int K, int N, int group,
+                        const uint32_t* planes, const void* scales_f16, const void* zeros_f16,
+                        void* y_f16, void* stream);
+
+/*
  * Host-buffer decode call (the end-to-end entry): x comes from HOST memory, the rank assignment and the VMM run in
  * one launch (grinqh_vmm_rank), y ends in HOST memory, all enqueued on `stream`.  x is staged with one
  * cudaMemcpyAsync (every CTA reads all of x for its rank selection).  With a pinned (page-locked) y_host the VMM's

@@ -56,6 +56,8 @@ _lib.grinqh_vmm_rank.restype = _i
 _lib.grinqh_vmm_rank.argtypes = [_vp, _i, _i, _i, _i, _vp, _vp, _vp, _vp, _vp, _vp, _sz, _vp]
 _lib.grinqh_vmm_rank_static.restype = _i
 _lib.grinqh_vmm_rank_static.argtypes = [_vp, _i, _i, _i, _i, _vp, _vp, _vp, _vp, _vp, _vp]
+_lib.grinqh_prefill_gemm.restype = _i
+_lib.grinqh_prefill_gemm.argtypes = [_vp, _i, _i, _i, _i, _vp, _vp, _vp, _vp, _vp]
 _lib.grinqh_static_scratch_bytes.restype = _sz
 _lib.grinqh_static_scratch_bytes.argtypes = []
 _lib.grinqh_pack_seg2.restype = _i
@@ -74,7 +76,7 @@ EXPORTS = ("grinqh_status_string", "grinqh_version", "grinqh_mix_to_counts", "gr
            "grinqh_calibrate_thresholds", "grinqh_vmm_workspace_bytes",
            "grinqh_vmm_workspace_init", "grinqh_vmm", "grinqh_vmm_thresholds", "grinqh_vmm_rank",
            "grinqh_vmm_main", "grinqh_vmm_reduce", "grinqh_decode_host", "grinqh_pack_seg2", "grinqh_vmm_rank_seg2",
-           "grinqh_static_scratch_bytes", "grinqh_vmm_rank_static")
+           "grinqh_static_scratch_bytes", "grinqh_vmm_rank_static", "grinqh_prefill_gemm")
 
 
 class GrinqhError(RuntimeError):
@@ -270,6 +272,19 @@ def grinqh_vmm_rank_static(x: torch.Tensor, counts, w: Packed, y: torch.Tensor, 
                                        w.planes.data_ptr(), w.scales.data_ptr(), w.zeros.data_ptr(),
                                        _dev(y, torch.float32, "y"), _stream(stream)), "grinqh_vmm_rank_static")
     return y
+
+
+def grinqh_prefill_gemm(X: torch.Tensor, w: Packed, Y: torch.Tensor | None = None, stream=None) -> torch.Tensor:
+    """Y [M, N] fp16 = X [M, K] fp16 . W_hat (b_max = 8), the unpack fused into a tcgen05 GEMM (prefill path)."""
+    M, K = X.shape
+    if K != w.K:
+        raise GrinqhError(f"X has K={K}, weight has K={w.K}")
+    if Y is None:
+        Y = torch.empty((M, w.N), dtype=torch.float16, device=X.device)
+    _check(_lib.grinqh_prefill_gemm(_dev(X, torch.float16, "X"), M, K, w.N, GROUP, w.planes.data_ptr(),
+                                    w.scales.data_ptr(), w.zeros.data_ptr(), _dev(Y, torch.float16, "Y"),
+                                    _stream(stream)), "grinqh_prefill_gemm")
+    return Y
 
 
 class PackedSeg2:

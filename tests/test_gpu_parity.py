@@ -633,3 +633,38 @@ def test_vmm_rank_seg2_full_size_sampled_columns(gq):
     sub_cols = np.array([remap[int(c) // 16] * 16 + int(c) % 16 for c in cols], np.int32)
     y_ref = oracle.vmm2(x, segs, s, z, oracle.assign(x, counts)["bits"], bmax, cols=sub_cols)
     _check_y(y[:, cols], y_ref)
+
+
+@pytest.mark.parametrize("M,K,N,seed", [(128, 128, 256, 0), (200, 512, 512, 2), (300, 2048, 768, 3), (1, 256, 256, 4),
+                                        (515, 1024, 1024, 5)])
+def test_prefill_gemm_fused_unpack_on_tensor_cores(gq, M, K, N, seed):
+    """Y = X . W_hat at b_max = 8 in one tcgen05 launch, the unpack fused into the
+    operand staging.  Oracle: x @ dequant(planes, s, z, 8) in fp64.  The kernel multiplies fp16 X by W_hat rounded once
+    to fp16 (relative 2^-11 per weight), accumulates in fp32 and rounds Y to fp16 (2^-11 per output): the relative L2
+    bound is 1e-3 and no element may be off by more than 2^-9 of the largest |y| of its row set."""
+    W = synth.make_weights(K, N, 0.02, seed)
+    W[:128, 0] = np.float16(0.25)                      # a constant group (s = 0)
+    rng = np.random.default_rng(seed + 900)
+    X = rng.standard_normal((M, K)).astype(np.float16)
+    X[0, :] = 0                                        # an all-zero token
+    planes, s, z = oracle.pack(W)
+    ref = X.astype(np.float64) @ oracle.dequant(planes, s, z, 8)
+    w = gq.grinqh_pack(_dev(W))
+    Y = torch.full((M, N), float("nan"), dtype=torch.float16, device="cuda")
+    gq.grinqh_prefill_gemm(_dev(X), w, Y)
+    torch.cuda.synchronize()
+    y = Y.cpu().numpy().astype(np.float64)
+    assert np.isfinite(y).all()
+    assert rel_l2(y, ref) <= 1e-3
+    assert np.abs(y - ref).max() <= 2.0 ** -9 * np.abs(ref).max()
+    assert not y[0].any()
+    # and it is the product on exactly the matrix grinqh_unpack writes: same inputs, fp32 accumulation on both sides
+    y_dense = (torch.from_numpy(X).cuda().float() @ gq.grinqh_unpack(w).float()).cpu().numpy()
+    assert np.abs(y - y_dense).max() <= 2.0 ** -9 * np.abs(ref).max()
+
+
+def test_prefill_gemm_rejects_unsupported_shapes(gq):
+    w = gq.grinqh_pack(_dev(synth.make_weights(128, 128, 0.02, 0)))   # N % 256 != 0
+    X = torch.zeros((4, 128), dtype=torch.float16, device="cuda")
+    with pytest.raises(gq.GrinqhError):
+        gq.grinqh_prefill_gemm(X, w)
