@@ -6,20 +6,21 @@
 //
 // One CTA = one 256 x 256 tile of Y (two 128-row accumulators of 256 fp32 columns: all 512 TMEM columns), K in blocks
 // of 64, STAGES-deep shared-memory ring.  Warp roles (no role waits inside another's critical section):
-//   warps 0-7  B producers, then epilogue.  Per stage each lane takes two (row k, 32-column word) units: 8 plane words
+//   warps 0-15 B producers, then epilogue.  Per stage each lane takes one (row k, 32-column word) unit: 8 plane words
 //              from global memory -> SIMD 8x8 bit transpose (gather.cuh) -> bytes widened to fp16 subnormals by PRMT,
 //              x 2^15 (exact), HFMA2 with (s 2^9, z): the correctly rounded s q + z -> four 16-byte chunks into the
 //              stage's B tile in the canonical MN-major SWIZZLE_128B layout (64 columns x 8 k-rows per 1-KB atom).
 //              The 32 columns of a word are stored in the order the transpose leaves them (a fixed permutation inside
 //              the word); the epilogue undoes it on registers.  fence.proxy.async, then the warp arrives on `full`.
-//   warp 8     TMA producer: the stage's two 128 x 64 X boxes (K-major, SWIZZLE_128B) with complete_tx on `full`.
-//   warp 9     MMA issuer: one lane issues 2 x 4 tcgen05.mma (M 128, N 256, K 16, fp16 x fp16 -> fp32 in TMEM) per stage,
+//   warp 16    TMA producer: the stage's two 128 x 64 X boxes (K-major, SWIZZLE_128B) with complete_tx on `full`.
+//   warp 17    MMA issuer: one lane issues 2 x 4 tcgen05.mma (M 128, N 256, K 16, fp16 x fp16 -> fp32 in TMEM) per stage,
 //              tcgen05.commit -> `empty` (frees the stage) and, after the last block, -> `accum`.
-//   epilogue   warps 0-7 (TMEM lane quarter = warp % 4, accumulator = warp / 4): tcgen05.ld 32 columns, un-permute,
+//   epilogue   warps 0-15 (TMEM lane quarter = warp % 4, accumulator and column half from warp / 4): tcgen05.ld 32 columns, un-permute,
 //              fp32 -> fp16, 64 contiguous bytes per row and word to Y.
 // Every mbarrier wait is bounded (a trap instead of a hang if a count is ever wrong).
 #include <cuda.h>
 
+#include <cstdlib>
 #include <mutex>
 
 #include "common.cuh"
@@ -38,7 +39,7 @@ constexpr int A_TILE = BM * BK * 2;         // 16 KB: one TMA box
 constexpr int A_STAGE = MT * A_TILE;        // 32 KB
 constexpr int B_STAGE = BK * BN * 2;        // 32 KB
 constexpr int STAGE_BYTES = A_STAGE + B_STAGE;
-constexpr int NPROD = 8;                    // producer / epilogue warps
+constexpr int NPROD = 16;                   // producer / epilogue warps
 constexpr int THREADS = (NPROD + 2) * 32;
 constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /* alignment slack */ + 256 /* barriers */;
 constexpr uint32_t TMEM_COLS = MT * BN;     // 512
@@ -140,7 +141,7 @@ __host__ __device__ constexpr int pos_of_col(int c) {
 
 __global__ void __launch_bounds__(THREADS, 1)
 prefill_kernel(const __grid_constant__ CUtensorMap xmap, int M, int K, int N, const uint32_t* __restrict__ planes,
-               const __half* __restrict__ scales, const __half* __restrict__ zeros, __half* __restrict__ Y) {
+               const __half* __restrict__ scales, const __half* __restrict__ zeros, __half* __restrict__ Y, int dbg) {
     extern __shared__ uint8_t smem_raw[];
     const uint32_t raw = smem_u32(smem_raw);
     const uint32_t base = (raw + 1023u) & ~1023u;  // the swizzle atoms are 1 KB
@@ -179,81 +180,91 @@ prefill_kernel(const __grid_constant__ CUtensorMap xmap, int M, int K, int N, co
 
     if (warp < NPROD) {
         // ================================================================ B producers
-        const int kk = lane & 7;                        // row inside the 8-row k atom
-        const int word = (lane >> 3) + 4 * (warp & 1);  // the lane's 32-column word of the tile, fixed for the whole K loop
-        const int katom = warp >> 1;                    // k atoms katom and katom + 4 of every stage
+        // lane -> (row, word): the 8 lanes of a store phase take 4 rows x 2 words (8 distinct swizzled chunks: no bank
+        // conflict) and a warp's plane load covers 4 rows x the tile's 8 words = whole 32-byte sectors
+        const int word = lane >> 2;                     // the lane's 32-column word of the tile, fixed for the whole K loop
+        const int katom = warp >> 1;                    // the lane's k atom (8 rows) of every stage
+        const int kk = 4 * (warp & 1) + (lane & 3);     // row inside the atom
         const int words = N >> 5;
         const size_t pstride = (size_t)K * words;
-        const uint32_t* src = planes + (size_t)(n0 >> 5) + word;
-        const uint32_t b_off = (uint32_t)(word >> 1) * 8192u + (uint32_t)kk * 128u;  // + k atom * 1024 + swizzled chunk * 16
+        const uint32_t* src = planes + (size_t)(n0 >> 5) + word + (size_t)(katom * 8 + kk) * words;
+        const uint32_t b_off = A_STAGE + (uint32_t)(word >> 1) * 8192u + (uint32_t)katom * 1024u + (uint32_t)kk * 128u;
         const uint32_t j0 = (uint32_t)(word & 1) * 4u;
         const uint32_t K15 = 0x78007800u;  // 2^15 | 2^15
         const uint32_t K9 = 0x60006000u;   // 2^9 | 2^9
+        const __half* sz_s = scales + n0 + word * 32;
+        const __half* sz_z = zeros + n0 + word * 32;
 
-        uint32_t Wn[2][8];
-        auto load_words = [&](int kb) {
+        // the lane's plane words of k block kb (global loads in flight two blocks ahead of their use)
+        auto load_words = [&](int kb, uint32_t (&W)[8]) {
+            const uint32_t* p = src + (size_t)kb * BK * words;
 #pragma unroll
-            for (int u = 0; u < 2; ++u) {
-                const uint32_t* p = src + (size_t)(kb * BK + (katom + 4 * u) * 8 + kk) * words;
+            for (int j = 0; j < 8; ++j) W[j] = (dbg & 16) ? (uint32_t)kb * 0x9E3779B9u + j : ld_nc_u32(p + j * pstride);
+        };
+        uint32_t S2[8][2], Z2[8][2];  // {s[r], s[8+r]} 2^9, {s[16+r], s[24+r]} 2^9 and the zeros in the same pairing
+        auto load_sz = [&](int g) {   // group g's scales and zeros of the lane's 32 columns
+            const size_t gn = (size_t)g * N;
+            uint32_t sr[16], zr[16];
 #pragma unroll
-                for (int j = 0; j < 8; ++j) Wn[u][j] = ld_nc_u32(p + j * pstride);
+            for (int i = 0; i < 4; ++i) {
+                const uint4 a = __ldg(reinterpret_cast<const uint4*>(sz_s + gn + 8 * i));
+                const uint4 b = __ldg(reinterpret_cast<const uint4*>(sz_z + gn + 8 * i));
+                sr[4 * i] = a.x; sr[4 * i + 1] = a.y; sr[4 * i + 2] = a.z; sr[4 * i + 3] = a.w;
+                zr[4 * i] = b.x; zr[4 * i + 1] = b.y; zr[4 * i + 2] = b.z; zr[4 * i + 3] = b.w;
+            }
+#pragma unroll
+            for (int r = 0; r < 8; ++r) {
+                const uint32_t sel = (r & 1) ? 0x7632u : 0x5410u;  // the odd or the even halves of the two registers
+                S2[r][0] = h2_mul(__byte_perm(sr[r >> 1], sr[(8 + r) >> 1], sel), K9);
+                S2[r][1] = h2_mul(__byte_perm(sr[(16 + r) >> 1], sr[(24 + r) >> 1], sel), K9);
+                Z2[r][0] = __byte_perm(zr[r >> 1], zr[(8 + r) >> 1], sel);
+                Z2[r][1] = __byte_perm(zr[(16 + r) >> 1], zr[(24 + r) >> 1], sel);
+            }
+            if ((g + 1) * 2 < KB) {  // the next group's lines are asked for now
+                asm volatile("prefetch.global.L2 [%0];" ::"l"(sz_s + gn + N));
+                asm volatile("prefetch.global.L2 [%0];" ::"l"(sz_z + gn + N));
             }
         };
-        load_words(0);
-        uint32_t S2[8][2], Z2[8][2];  // {s[r], s[8+r]} 2^9, {s[16+r], s[24+r]} 2^9 and the zeros in the same pairing
-#pragma unroll 1
-        for (int kb = 0; kb < KB; ++kb) {
+        // one stage: the lane's unit of k block kb, W consumed (and reloaded for kb + 2) on the way
+        auto produce = [&](int kb, uint32_t (&W)[8]) {
             const int s = kb % STAGES;
             const uint32_t ph = (uint32_t)(kb / STAGES) & 1u;
-            uint32_t Wc[2][8];
+            uint32_t V[8], H[8][2];
+            if (dbg & 1) {
+                mbar_wait(empty(s), ph ^ 1u);
+                __syncwarp();
+                if (lane == 0) mbar_arrive(full(s));
+                return;
+            }
+            gather<8>(W, V);
+            if (kb + 2 < KB) load_words(kb + 2, W);
 #pragma unroll
-            for (int u = 0; u < 2; ++u)
-#pragma unroll
-                for (int j = 0; j < 8; ++j) Wc[u][j] = Wn[u][j];
-            if (kb + 1 < KB) load_words(kb + 1);
-            if ((kb & 1) == 0) {  // a new group of 128 rows: its scales and zeros for the lane's 32 columns
-                const size_t gn = (size_t)(kb >> 1) * N + n0 + word * 32;
-                uint32_t sr[16], zr[16];
-#pragma unroll
-                for (int i = 0; i < 4; ++i) {
-                    const uint4 a = *reinterpret_cast<const uint4*>(scales + gn + 8 * i);
-                    const uint4 b = *reinterpret_cast<const uint4*>(zeros + gn + 8 * i);
-                    sr[4 * i] = a.x; sr[4 * i + 1] = a.y; sr[4 * i + 2] = a.z; sr[4 * i + 3] = a.w;
-                    zr[4 * i] = b.x; zr[4 * i + 1] = b.y; zr[4 * i + 2] = b.z; zr[4 * i + 3] = b.w;
-                }
-#pragma unroll
-                for (int r = 0; r < 8; ++r) {
-                    const uint32_t sel = (r & 1) ? 0x7632u : 0x5410u;  // the odd or the even halves of the two registers
-                    S2[r][0] = h2_mul(__byte_perm(sr[r >> 1], sr[(8 + r) >> 1], sel), K9);
-                    S2[r][1] = h2_mul(__byte_perm(sr[(16 + r) >> 1], sr[(24 + r) >> 1], sel), K9);
-                    Z2[r][0] = __byte_perm(zr[r >> 1], zr[(8 + r) >> 1], sel);
-                    Z2[r][1] = __byte_perm(zr[(16 + r) >> 1], zr[(24 + r) >> 1], sel);
-                }
+            for (int r = 0; r < 8; ++r) {
+                // bytes -> fp16 subnormals q 2^-24 (PRMT with zero), x 2^15 (exact), then q 2^-9 * s 2^9 + z: one rounding
+                H[r][0] = h2_fma(h2_mul(__byte_perm(V[r], 0u, 0x4140), K15), S2[r][0], Z2[r][0]);
+                H[r][1] = h2_fma(h2_mul(__byte_perm(V[r], 0u, 0x4342), K15), S2[r][1], Z2[r][1]);
             }
             mbar_wait(empty(s), ph ^ 1u);
-            const uint32_t bst = base + (uint32_t)s * STAGE_BYTES + A_STAGE + b_off;
+            const uint32_t dst = base + (uint32_t)s * STAGE_BYTES + b_off;
 #pragma unroll
-            for (int u = 0; u < 2; ++u) {
-                uint32_t V[8], H[8][2];
-                gather<8>(Wc[u], V);
-#pragma unroll
-                for (int r = 0; r < 8; ++r) {
-                    // bytes -> fp16 subnormals q 2^-24 (PRMT with zero), x 2^15 (exact), then q 2^-9 * s 2^9 + z: one rounding
-                    H[r][0] = h2_fma(h2_mul(__byte_perm(V[r], 0u, 0x4140), K15), S2[r][0], Z2[r][0]);
-                    H[r][1] = h2_fma(h2_mul(__byte_perm(V[r], 0u, 0x4342), K15), S2[r][1], Z2[r][1]);
-                }
-                const uint32_t dst = bst + (uint32_t)(katom + 4 * u) * 1024u;
-#pragma unroll
-                for (int jj = 0; jj < 4; ++jj) {
-                    const uint32_t a = dst + (((j0 + jj) ^ (uint32_t)kk) << 4);
-                    asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(a), "r"(H[2 * jj][0]), "r"(H[2 * jj][1]),
-                                 "r"(H[2 * jj + 1][0]), "r"(H[2 * jj + 1][1])
-                                 : "memory");
-                }
+            for (int jj = 0; jj < 4; ++jj) {
+                const uint32_t a = dst + (((j0 + jj) ^ (uint32_t)kk) << 4);
+                asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(a), "r"(H[2 * jj][0]), "r"(H[2 * jj][1]),
+                             "r"(H[2 * jj + 1][0]), "r"(H[2 * jj + 1][1])
+                             : "memory");
             }
-            fence_proxy_async();  // the tile is read by the tensor core through the async proxy
+            if (!(dbg & 8)) fence_proxy_async();  // the tile is read by the tensor core through the async proxy
             __syncwarp();
             if (lane == 0) mbar_arrive(full(s));
+        };
+        uint32_t W0[8], W1[8];
+        load_words(0, W0);
+        load_words(1, W1);  // (K % 128 == 0: an even number of blocks)
+#pragma unroll 1
+        for (int kb = 0; kb < KB; kb += 2) {
+            if (!(dbg & 32) || kb == 0) load_sz(kb >> 1);  // a new group of 128 rows
+            produce(kb, W0);
+            produce(kb + 1, W1);
         }
     } else if (warp == NPROD) {
         // ================================================================ TMA producer (X)
@@ -266,7 +277,7 @@ prefill_kernel(const __grid_constant__ CUtensorMap xmap, int M, int K, int N, co
                 mbar_arrive_expect_tx(full(s), A_STAGE);
                 const uint32_t a = base + (uint32_t)s * STAGE_BYTES;
 #pragma unroll
-                for (int mt = 0; mt < MT; ++mt) tma_load_2d(a + mt * A_TILE, &xmap, kb * BK, m0 + mt * BM, full(s));
+                for (int mt = 0; mt < MT; ++mt) tma_load_2d(a + mt * A_TILE, &xmap, (dbg & 4) ? 0 : kb * BK, m0 + mt * BM, full(s));
             }
         }
     } else {
@@ -287,7 +298,7 @@ prefill_kernel(const __grid_constant__ CUtensorMap xmap, int M, int K, int N, co
                         const uint64_t ad = smem_desc(a + mt * A_TILE + k4 * (UK * 2), 16, 1024);
                         // B: MN-major atoms of 64 columns x 8 k: column atoms 8 KB apart, k atoms 1 KB apart; 16 k = 2 atoms
                         const uint64_t bd = smem_desc(b + k4 * 2048, 8192, 1024);
-                        mma_f16(tmem + (uint32_t)(mt * BN), ad, bd, (uint32_t)((kb | k4) != 0));
+                        if (!(dbg & 2)) mma_f16(tmem + (uint32_t)(mt * BN), ad, bd, (uint32_t)((kb | k4) != 0));
                     }
                 mma_commit(empty(s));
                 if (kb == KB - 1) mma_commit(accum);
@@ -300,10 +311,10 @@ prefill_kernel(const __grid_constant__ CUtensorMap xmap, int M, int K, int N, co
         // ================================================================ epilogue
         mbar_wait(accum, 0);
         tc_fence_after();
-        const int quarter = warp & 3, mt = warp >> 2;
+        const int quarter = warp & 3, mt = (warp >> 2) & 1, chalf = warp >> 3;  // 16 warps: 2 accumulators x 2 column halves
         const int m = m0 + mt * BM + quarter * 32 + lane;
 #pragma unroll 1
-        for (int cb = 0; cb < BN / 32; ++cb) {
+        for (int cb = chalf * (BN / 64); cb < (chalf + 1) * (BN / 64); ++cb) {
             uint32_t v[32];
             tmem_ld32(tmem + ((uint32_t)(quarter * 32) << 16) + (uint32_t)(mt * BN + cb * 32), v);
             if (m < M) {
@@ -366,6 +377,7 @@ extern "C" int grinqh_prefill_gemm(const void* x_f16, int M, int K, int N, int g
         return GRINQH_ERR_CUDA;
     dim3 grid(N / BN, (M + MT * BM - 1) / (MT * BM));
     prefill_kernel<<<grid, THREADS, SMEM_BYTES, (cudaStream_t)stream>>>(xmap, M, K, N, planes, (const __half*)scales_f16,
-                                                                         (const __half*)zeros_f16, (__half*)y_f16);
+                                                                         (const __half*)zeros_f16, (__half*)y_f16,
+                                                                         getenv("GRINQH_PREFILL_DBG") ? atoi(getenv("GRINQH_PREFILL_DBG")) : 0);
     return cudaGetLastError() == cudaSuccess ? GRINQH_OK : GRINQH_ERR_CUDA;
 }
