@@ -52,7 +52,7 @@ def _args():
     ap.add_argument("--seed", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sweep", action="store_true", help="configs 3 and 5: per-VMM latency vs average bits (not the contract line)")
-    ap.add_argument("--prefill", action="store_true", help="f3 (part): grinqh_unpack + dense library GEMM timings")
+    ap.add_argument("--prefill", action="store_true", help="f3: fused tcgen05 prefill GEMM against grinqh_unpack + dense library GEMM")
     ap.add_argument("--decode-step", action="store_true", help="config 4: 32-layer decode step in one CUDA graph")
     ap.add_argument("--no-split", action="store_true", help="skip the one-launch-per-projection variant")
     ap.add_argument("--seg2", action="store_true", help="f2: 2-bit-segment store against the 1-bit plane store (A/B)")
@@ -67,6 +67,17 @@ def _peaks():
         except Exception:
             pass
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def _tensor_peak():
+    """Dense 16-bit tensor peak for a kernel timed alone (burst figure of MEASURED_PEAKS.json; fp16 = bf16 rate)."""
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["bf16_tflops"]), "measured (MEASURED_PEAKS.json bf16_tflops, burst)"
+        except Exception:
+            pass
+    return 2250.0, "fallback (nominal dense bf16 2.25 PFLOP/s)"
 
 
 def alg_bytes(K, N, T, sum_bits):
@@ -657,12 +668,26 @@ def run_prefill(args):
 
         us_unpack = timed(lambda: gq.grinqh_unpack(w, out), 20)
         us_gemm = timed(lambda: torch.matmul(X, out), 10)
+        Y = torch.empty((tokens, N), device=dev, dtype=torch.float16)
+        us_fused = timed(lambda: gq.grinqh_prefill_gemm(X, w, Y), 10)   # f3: unpack fused into the tcgen05 GEMM
+        same = bool(torch.equal(Y, torch.matmul(X, out)))
+        tf_peak, tf_src = _tensor_peak()
+        flops = 2 * tokens * K * N
         print("PREFILL " + json.dumps({"K": K, "N": N, "tokens": tokens, "us_unpack": us_unpack,
                                        "unpack_GBps": K * N * 3 / us_unpack / 1e3,
                                        "unpack_frac_of_measured_hbm": K * N * 3 / us_unpack / 1e3 / peak,
                                        "us_dense_gemm_fp16_torch": us_gemm,
-                                       "gemm_TFLOPs": 2 * tokens * K * N / us_gemm / 1e6,
-                                       "unpack_over_gemm": us_unpack / us_gemm}), flush=True)
+                                       "gemm_TFLOPs": flops / us_gemm / 1e6,
+                                       "unpack_over_gemm": us_unpack / us_gemm,
+                                       "us_fused_prefill_gemm": us_fused,
+                                       "fused_TFLOPs": flops / us_fused / 1e6,
+                                       "fused_over_unpack_plus_gemm": us_fused / (us_unpack + us_gemm),
+                                       "fused_equals_library_path_bitwise": same,
+                                       "roofline": {"bound": "tensor", "achieved": flops / us_fused / 1e6, "peak": tf_peak,
+                                                    "unit": "TFLOP/s", "frac": flops / us_fused / 1e6 / tf_peak,
+                                                    "peak_source": tf_src, "kernel": "prefill_kernel (tcgen05, fp16 dense)"}}),
+              flush=True)
+        del Y
         del W, w, out, X
 
 

@@ -40,8 +40,12 @@ constexpr int A_STAGE = MT * A_TILE;        // 32 KB
 constexpr int B_STAGE = BK * BN * 2;        // 32 KB
 constexpr int STAGE_BYTES = A_STAGE + B_STAGE;
 constexpr int NPROD = 16;                   // producer / epilogue warps
-constexpr int THREADS = (NPROD + 2) * 32;
-constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /* alignment slack */ + 256 /* barriers */;
+constexpr int THREADS = (NPROD + 3) * 32;   // + TMA warp for X, TMA warp for the planes, MMA warp
+constexpr int RAW_BYTES = 8 * BK * (BN / 32) * 4;  // 16 KB: the stage's plane words, [plane][row][8 words]
+constexpr int RAW_BUFS = 2;
+constexpr int RAW_OFF = STAGES * STAGE_BYTES;
+constexpr int BAR_OFF = RAW_OFF + RAW_BUFS * RAW_BYTES;
+constexpr int SMEM_BYTES = BAR_OFF + 1024 /* alignment slack */ + 256 /* barriers */;
 constexpr uint32_t TMEM_COLS = MT * BN;     // 512
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -79,6 +83,13 @@ __device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map
     asm volatile(
         "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];" ::"r"(dst),
         "l"(map), "r"(c0), "r"(c1), "r"(bar)
+        : "memory");
+}
+
+__device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* map, int c0, int c1, int c2, uint32_t bar) {
+    asm volatile(
+        "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];" ::"r"(dst),
+        "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(bar)
         : "memory");
 }
 
@@ -140,23 +151,35 @@ __host__ __device__ constexpr int pos_of_col(int c) {
 }
 
 __global__ void __launch_bounds__(THREADS, 1)
-prefill_kernel(const __grid_constant__ CUtensorMap xmap, int M, int K, int N, const uint32_t* __restrict__ planes,
-               const __half* __restrict__ scales, const __half* __restrict__ zeros, __half* __restrict__ Y, int dbg) {
+prefill_kernel(const __grid_constant__ CUtensorMap xmap, const __grid_constant__ CUtensorMap pmap, int M, int K, int N,
+               const __half* __restrict__ scales, const __half* __restrict__ zeros, __half* __restrict__ Y, int dbg_arg) {
+#ifdef GQ_PREFILL_DBG
+    const int dbg = dbg_arg;  // measurement build only: legs of the kernel switched off (results are then wrong on purpose)
+#else
+    constexpr int dbg = 0;
+    (void)dbg_arg;
+#endif
     extern __shared__ uint8_t smem_raw[];
     const uint32_t raw = smem_u32(smem_raw);
     const uint32_t base = (raw + 1023u) & ~1023u;  // the swizzle atoms are 1 KB
     uint8_t* sm = smem_raw + (base - raw);
-    const uint32_t bars = base + STAGES * STAGE_BYTES;
+    const uint32_t bars = base + BAR_OFF;
     auto full = [&](int s) { return bars + 8u * s; };
     auto empty = [&](int s) { return bars + 8u * (STAGES + s); };
     const uint32_t accum = bars + 8u * (2 * STAGES);
-    volatile uint32_t* tmem_slot = reinterpret_cast<volatile uint32_t*>(sm + STAGES * STAGE_BYTES + 8 * (2 * STAGES + 1));
+    auto rawfull = [&](int i) { return bars + 8u * (2 * STAGES + 2 + i); };
+    auto rawempty = [&](int i) { return bars + 8u * (2 * STAGES + 2 + RAW_BUFS + i); };
+    volatile uint32_t* tmem_slot = reinterpret_cast<volatile uint32_t*>(sm + BAR_OFF + 8 * (2 * STAGES + 1));
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int n0 = blockIdx.x * BN, m0 = blockIdx.y * (MT * BM);
     const int KB = K / BK;
 
-    if (warp == NPROD + 1 && lane == 0) {
+    if (warp == NPROD + 2 && lane == 0) {
+        for (int i = 0; i < RAW_BUFS; ++i) {
+            mbar_init(rawfull(i), 1);       // the plane TMA thread's arrive.expect_tx
+            mbar_init(rawempty(i), NPROD);  // every producer warp has taken its words
+        }
         for (int s = 0; s < STAGES; ++s) {
             mbar_init(full(s), NPROD + 1);  // the producer warps + the TMA thread's arrive.expect_tx
             mbar_init(empty(s), 1);         // one tcgen05.commit
@@ -166,6 +189,7 @@ prefill_kernel(const __grid_constant__ CUtensorMap xmap, int M, int K, int N, co
         fence_proxy_async();
     }
     if (warp == NPROD && lane == 0) asm volatile("prefetch.tensormap [%0];" ::"l"(&xmap) : "memory");
+    if (warp == NPROD + 1 && lane == 0) asm volatile("prefetch.tensormap [%0];" ::"l"(&pmap) : "memory");
     if (warp == 0) {  // the whole warp allocates all 512 TMEM columns (one CTA per SM: nobody else asks)
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(
                          bars + 8u * (2 * STAGES + 1)),
@@ -185,9 +209,8 @@ prefill_kernel(const __grid_constant__ CUtensorMap xmap, int M, int K, int N, co
         const int word = lane >> 2;                     // the lane's 32-column word of the tile, fixed for the whole K loop
         const int katom = warp >> 1;                    // the lane's k atom (8 rows) of every stage
         const int kk = 4 * (warp & 1) + (lane & 3);     // row inside the atom
-        const int words = N >> 5;
-        const size_t pstride = (size_t)K * words;
-        const uint32_t* src = planes + (size_t)(n0 >> 5) + word + (size_t)(katom * 8 + kk) * words;
+        // the lane's word of plane j in the raw tile [plane][row][8 words]: the 32 lanes of a warp hit 32 distinct banks
+        const uint32_t raw_off = RAW_OFF + (uint32_t)(katom * 8 + kk) * 32u + (uint32_t)word * 4u;
         const uint32_t b_off = A_STAGE + (uint32_t)(word >> 1) * 8192u + (uint32_t)katom * 1024u + (uint32_t)kk * 128u;
         const uint32_t j0 = (uint32_t)(word & 1) * 4u;
         const uint32_t K15 = 0x78007800u;  // 2^15 | 2^15
@@ -195,12 +218,6 @@ prefill_kernel(const __grid_constant__ CUtensorMap xmap, int M, int K, int N, co
         const __half* sz_s = scales + n0 + word * 32;
         const __half* sz_z = zeros + n0 + word * 32;
 
-        // the lane's plane words of k block kb (global loads in flight two blocks ahead of their use)
-        auto load_words = [&](int kb, uint32_t (&W)[8]) {
-            const uint32_t* p = src + (size_t)kb * BK * words;
-#pragma unroll
-            for (int j = 0; j < 8; ++j) W[j] = (dbg & 16) ? (uint32_t)kb * 0x9E3779B9u + j : ld_nc_u32(p + j * pstride);
-        };
         uint32_t S2[8][2], Z2[8][2];  // {s[r], s[8+r]} 2^9, {s[16+r], s[24+r]} 2^9 and the zeros in the same pairing
         auto load_sz = [&](int g) {   // group g's scales and zeros of the lane's 32 columns
             const size_t gn = (size_t)g * N;
@@ -225,19 +242,25 @@ prefill_kernel(const __grid_constant__ CUtensorMap xmap, int M, int K, int N, co
                 asm volatile("prefetch.global.L2 [%0];" ::"l"(sz_z + gn + N));
             }
         };
-        // one stage: the lane's unit of k block kb, W consumed (and reloaded for kb + 2) on the way
-        auto produce = [&](int kb, uint32_t (&W)[8]) {
+        // one stage: the lane's unit of k block kb
+        auto produce = [&](int kb) {
             const int s = kb % STAGES;
             const uint32_t ph = (uint32_t)(kb / STAGES) & 1u;
-            uint32_t V[8], H[8][2];
+            const int rb = kb % RAW_BUFS;
+            uint32_t W[8], V[8], H[8][2];
+            mbar_wait(rawfull(rb), (uint32_t)(kb / RAW_BUFS) & 1u);  // the stage's plane words have landed (TMA)
+#pragma unroll
+            for (int j = 0; j < 8; ++j)
+                asm volatile("ld.shared.b32 %0, [%1];" : "=r"(W[j]) : "r"(base + raw_off + (uint32_t)rb * RAW_BYTES + (uint32_t)j * 2048u));
+            gather<8>(W, V);
+            __syncwarp();
+            if (lane == 0) mbar_arrive(rawempty(rb));  // the warp's loads have returned (their values are consumed above)
             if (dbg & 1) {
                 mbar_wait(empty(s), ph ^ 1u);
                 __syncwarp();
-                if (lane == 0) mbar_arrive(full(s));
+                if (lane == 0) mbar_arrive(full(s) + (V[0] == 0x12345678u ? 1u : 0u));
                 return;
             }
-            gather<8>(W, V);
-            if (kb + 2 < KB) load_words(kb + 2, W);
 #pragma unroll
             for (int r = 0; r < 8; ++r) {
                 // bytes -> fp16 subnormals q 2^-24 (PRMT with zero), x 2^15 (exact), then q 2^-9 * s 2^9 + z: one rounding
@@ -257,14 +280,10 @@ prefill_kernel(const __grid_constant__ CUtensorMap xmap, int M, int K, int N, co
             __syncwarp();
             if (lane == 0) mbar_arrive(full(s));
         };
-        uint32_t W0[8], W1[8];
-        load_words(0, W0);
-        load_words(1, W1);  // (K % 128 == 0: an even number of blocks)
 #pragma unroll 1
-        for (int kb = 0; kb < KB; kb += 2) {
-            if (!(dbg & 32) || kb == 0) load_sz(kb >> 1);  // a new group of 128 rows
-            produce(kb, W0);
-            produce(kb + 1, W1);
+        for (int kb = 0; kb < KB; ++kb) {
+            if ((kb & 1) == 0) load_sz(kb >> 1);  // a new group of 128 rows
+            produce(kb);
         }
     } else if (warp == NPROD) {
         // ================================================================ TMA producer (X)
@@ -278,6 +297,19 @@ prefill_kernel(const __grid_constant__ CUtensorMap xmap, int M, int K, int N, co
                 const uint32_t a = base + (uint32_t)s * STAGE_BYTES;
 #pragma unroll
                 for (int mt = 0; mt < MT; ++mt) tma_load_2d(a + mt * A_TILE, &xmap, (dbg & 4) ? 0 : kb * BK, m0 + mt * BM, full(s));
+            }
+        }
+    } else if (warp == NPROD + 1) {
+        // ================================================================ TMA producer (plane words): one 3-D box per k block,
+        // 8 planes x 64 rows x 32 bytes, into the raw double buffer; no L1 miss tracking, no registers, no address arithmetic
+        if (lane == 0) {
+#pragma unroll 1
+            for (int kb = 0; kb < KB; ++kb) {
+                const int rb = kb % RAW_BUFS;
+                mbar_wait(rawempty(rb), ((uint32_t)(kb / RAW_BUFS) & 1u) ^ 1u);
+                mbar_arrive_expect_tx(rawfull(rb), RAW_BYTES);
+                if (!(dbg & 16)) tma_load_3d(base + RAW_OFF + (uint32_t)rb * RAW_BYTES, &pmap, n0 >> 5, kb * BK, 0, rawfull(rb));
+                else asm volatile("mbarrier.complete_tx.relaxed.cta.shared::cta.b64 [%0], %1;" ::"r"(rawfull(rb)), "r"((uint32_t)RAW_BYTES) : "memory");
             }
         }
     } else {
@@ -373,11 +405,23 @@ extern "C" int grinqh_prefill_gemm(const void* x_f16, int M, int K, int N, int g
             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
         return GRINQH_ERR_CUDA;
+    CUtensorMap pmap;  // planes as [8 planes][K rows][N/32 words] u32, box = 8 words x 64 rows x 8 planes
+    const cuuint64_t pdims[3] = {(cuuint64_t)(N / 32), (cuuint64_t)K, 8};
+    const cuuint64_t pstrides[2] = {(cuuint64_t)(N / 8), (cuuint64_t)K * (cuuint64_t)(N / 8)};
+    const cuuint32_t pbox[3] = {(cuuint32_t)(BN / 32), (cuuint32_t)BK, 8};
+    const cuuint32_t pestr[3] = {1, 1, 1};
+    if (enc(&pmap, CU_TENSOR_MAP_DATA_TYPE_UINT32, 3, const_cast<uint32_t*>(planes), pdims, pstrides, pbox, pestr,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+        return GRINQH_ERR_CUDA;
+    int dbg = 0;
+#ifdef GQ_PREFILL_DBG  // GQ_NVCC_EXTRA=-DGQ_PREFILL_DBG: 1 no unpack, 2 no MMA, 4 X from k = 0, 8 no proxy fence, 16 no plane loads
+    if (const char* e = getenv("GRINQH_PREFILL_DBG")) dbg = atoi(e);
+#endif
     if (cudaFuncSetAttribute(prefill_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES) != cudaSuccess)
         return GRINQH_ERR_CUDA;
     dim3 grid(N / BN, (M + MT * BM - 1) / (MT * BM));
-    prefill_kernel<<<grid, THREADS, SMEM_BYTES, (cudaStream_t)stream>>>(xmap, M, K, N, planes, (const __half*)scales_f16,
-                                                                         (const __half*)zeros_f16, (__half*)y_f16,
-                                                                         getenv("GRINQH_PREFILL_DBG") ? atoi(getenv("GRINQH_PREFILL_DBG")) : 0);
+    prefill_kernel<<<grid, THREADS, SMEM_BYTES, (cudaStream_t)stream>>>(xmap, pmap, M, K, N, (const __half*)scales_f16,
+                                                                         (const __half*)zeros_f16, (__half*)y_f16, dbg);
     return cudaGetLastError() == cudaSuccess ? GRINQH_OK : GRINQH_ERR_CUDA;
 }
