@@ -7,13 +7,16 @@
 // One CTA = one 256 x 256 tile of Y (two 128-row accumulators of 256 fp32 columns: all 512 TMEM columns), K in blocks
 // of 64, STAGES-deep shared-memory ring.  Warp roles (no role waits inside another's critical section):
 //   warps 0-15 B producers, then epilogue.  Per stage each lane takes one (row k, 32-column word) unit: 8 plane words
-//              from global memory -> SIMD 8x8 bit transpose (gather.cuh) -> bytes widened to fp16 subnormals by PRMT,
+//              from the raw buffer (LDS, conflict-free) -> SIMD 8x8 bit transpose (gather.cuh) -> bytes widened to fp16 subnormals by PRMT,
 //              x 2^15 (exact), HFMA2 with (s 2^9, z): the correctly rounded s q + z -> four 16-byte chunks into the
 //              stage's B tile in the canonical MN-major SWIZZLE_128B layout (64 columns x 8 k-rows per 1-KB atom).
 //              The 32 columns of a word are stored in the order the transpose leaves them (a fixed permutation inside
 //              the word); the epilogue undoes it on registers.  fence.proxy.async, then the warp arrives on `full`.
 //   warp 16    TMA producer: the stage's two 128 x 64 X boxes (K-major, SWIZZLE_128B) with complete_tx on `full`.
-//   warp 17    MMA issuer: one lane issues 2 x 4 tcgen05.mma (M 128, N 256, K 16, fp16 x fp16 -> fp32 in TMEM) per stage,
+//   warp 17    TMA producer for the plane words: one 3-D box per k block (8 planes x 64 rows x 32 bytes) into a raw double
+//              buffer [plane][row][8 words] (`rawfull` / `rawempty`).  Per-lane global loads stalled the producers: 1024
+//              sectors in flight per SM are more than the L1 miss path tracks (profiles/r02_prefill.md).
+//   warp 18    MMA issuer: one lane issues 2 x 4 tcgen05.mma (M 128, N 256, K 16, fp16 x fp16 -> fp32 in TMEM) per stage,
 //              tcgen05.commit -> `empty` (frees the stage) and, after the last block, -> `accum`.
 //   epilogue   warps 0-15 (TMEM lane quarter = warp % 4, accumulator and column half from warp / 4): tcgen05.ld 32 columns, un-permute,
 //              fp32 -> fp16, 64 contiguous bytes per row and word to Y.
