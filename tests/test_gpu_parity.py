@@ -663,6 +663,33 @@ def test_prefill_gemm_fused_unpack_on_tensor_cores(gq, M, K, N, seed):
     assert np.abs(y - y_dense).max() <= 2.0 ** -9 * np.abs(ref).max()
 
 
+def test_prefill_gemm_full_size_sampled(gq):
+    """The shape bench.py --prefill times (3000 tokens x 4096 x 14336, the paper's 3000:1 benchmark):
+    sampled rows x sampled columns recomputed by the oracle in fp64 (columns are independent: only the 32-column blocks
+    that contain sampled columns are packed on the host)."""
+    M, K, N = 3000, 4096, 14336
+    g = torch.Generator(device="cuda")
+    g.manual_seed(4242)
+    Wd = (torch.randn((K, N), generator=g, device="cuda", dtype=torch.float32) * 0.02).to(torch.float16)
+    Xd = torch.randn((M, K), generator=g, device="cuda", dtype=torch.float32).to(torch.float16)
+    w = gq.grinqh_pack(Wd)
+    Y = gq.grinqh_prefill_gemm(Xd, w)
+    torch.cuda.synchronize()
+    rng = np.random.default_rng(7)
+    cols = np.unique(np.concatenate([np.arange(0, 32), np.arange(N - 32, N), rng.integers(0, N, 96)])).astype(np.int64)
+    rows = np.unique(np.concatenate([[0, 127, 128, 255, 256, 2943, 2944, 2999], rng.integers(0, M, 24)])).astype(np.int64)
+    blocks = np.unique(cols // 32)
+    Wh = Wd[:, torch.from_numpy(np.concatenate([np.arange(b * 32, (b + 1) * 32) for b in blocks])).cuda()].cpu().numpy()
+    planes, s, z = oracle.pack(np.ascontiguousarray(Wh))
+    assert np.array_equal(w.planes[:, :, torch.from_numpy(blocks).cuda()].cpu().numpy().view(np.uint32), planes)
+    remap = {int(b): i for i, b in enumerate(blocks)}
+    sub = np.array([remap[int(c) // 32] * 32 + int(c) % 32 for c in cols])
+    ref = Xd[torch.from_numpy(rows).cuda()].cpu().numpy().astype(np.float64) @ oracle.dequant(planes, s, z, 8)[:, sub]
+    y = Y[torch.from_numpy(rows).cuda()][:, torch.from_numpy(cols).cuda()].cpu().numpy().astype(np.float64)
+    assert rel_l2(y, ref) <= 1e-3
+    assert np.abs(y - ref).max() <= 2.0 ** -9 * np.abs(ref).max()
+
+
 def test_prefill_gemm_rejects_unsupported_shapes(gq):
     w = gq.grinqh_pack(_dev(synth.make_weights(128, 128, 0.02, 0)))   # N % 256 != 0
     X = torch.zeros((4, 128), dtype=torch.float16, device="cuda")
