@@ -428,7 +428,7 @@ def run_native(args):
                      "traffic_source": (f"dram__bytes_read.sum + dram__bytes_write.sum of the step's launches, committed "
                                         f"ncu --set full capture (profiles/r02_traffic.json, taken on {traffic_on})"
                                         if traffic else "no committed capture for this mix"),
-                     "kernel": f"vmm_kernel<T=1, MODE_RANK> ({len(fused)} launches per step = the whole step)",
+                     "kernel": f"items::vmm_items_kernel<1, 16, true> in rank mode, grinqh_vmm_rank ({len(fused)} launches per step = the whole step)",
                      "alg_bytes_per_step": step_bytes, "plane_bytes_per_step": plane_bytes,
                      "us_per_step_vmm_on_ready_schedules": us_sched,
                      "frac_vmm_on_ready_schedules": step_bytes / (us_sched * 1e-6) / 1e9 / peak,
