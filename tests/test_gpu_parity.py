@@ -695,3 +695,29 @@ def test_prefill_gemm_rejects_unsupported_shapes(gq):
     X = torch.zeros((4, 128), dtype=torch.float16, device="cuda")
     with pytest.raises(gq.GrinqhError):
         gq.grinqh_prefill_gemm(X, w)
+
+
+def test_second_device_when_present(gq):
+    """the kernels' shared-memory attribute and the static scratch address are per device.  With two or more
+    GPUs the same calls on device 1 must work and return device 0's bits (skipped on a one-GPU box)."""
+    if torch.cuda.device_count() < 2:
+        pytest.skip("one GPU")
+    T, K, N = 2, 1024, 2080
+    W = synth.make_weights(K, N, 0.02, 3)
+    x = synth.make_x(T, K, 3, "student_t")
+    counts = gq.grinqh_mix_to_counts(K, synth.MIXES["4"])
+    ys = []
+    for d in (0, 1):
+        with torch.cuda.device(d):
+            dev = torch.device("cuda", d)
+            w = gq.grinqh_pack(torch.from_numpy(W).to(dev))
+            xd = torch.from_numpy(x).to(dev)
+            y = gq.grinqh_vmm_rank(xd, counts, w)
+            y2 = torch.empty_like(y)
+            gq.grinqh_vmm_rank_static(xd, counts, w, y2)
+            a = gq.grinqh_assign(xd, counts)
+            y3 = gq.grinqh_vmm(w, a)
+            torch.cuda.synchronize(dev)
+            assert torch.equal(y, y2) and torch.equal(y, y3)
+            ys.append(y.cpu().numpy())
+    assert np.array_equal(ys[0], ys[1])
