@@ -99,7 +99,9 @@ static inline VmmPlan vmm_plan(int T, int K, int N) {
             if (Sx > sx_max) Sx = sx_max;
             const int ipw = (I + vw * Sx - 1) / (vw * Sx);
             Sx = (I + vw * ipw - 1) / (vw * ipw);
-            const double cost = ipw * (112.0 / Q + 6.0) + 4.0 + 0.12 * Sx;  // + second pass, in row units (~0.45 us)
+            // (item overhead 12 rows: measured on this kernel — a sweep of the constant over the configs' shapes, 6 -> 12:
+            // layer step 83.9 -> 82.5 us, the 70B shapes up to 13 % faster in the rank form; profiles/r02_kernels.md)
+            const double cost = ipw * (112.0 / Q + 12.0) + 4.0 + 0.12 * Sx;  // + second pass, in row units (~0.45 us)
             if (cost < best_cost - 1e-9) {
                 best_cost = cost;
                 best = VmmPlan{CT, Q, Sx, ipw, vw};
